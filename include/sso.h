@@ -1,0 +1,154 @@
+/*
+ * sso.h -- C ABI of the B200-native Fourier split-operator library.
+ *
+ * One call of sso_step advances a complex wavefunction (Schroedinger, 1 component)
+ * or a Dirac spinor (2 or 4 components) on a regular periodic lattice by `nsteps`
+ * Fourier split-operator time steps
+ *
+ *     w(t+tau) = U_A1(1/2) F^-1{ U~_A2(1) F{ U_A1(1/2) w(t) } }
+ *
+ * i.e. PAPER.md:71 (eq. 7, Strang factorisation) in the Fourier form of
+ * PAPER.md:76 (eq. 8), on the lattice of PAPER.md:80 (all line numbers refer to
+ * the paper text, Bauke & Keitel, arXiv:1012.3911).  U_A1 is the position-space
+ * phase exp(-i Vbar tau/2) of PAPER.md:98 (eq. 11) / 165 (eq. 22); U~_A2 is, in
+ * momentum space, the phase exp(-i tau (k - q Abar)^2 / 2m) of PAPER.md:107
+ * (eq. 13) for Schroedinger and the per-k 2x2 / 4x4 unitary
+ * exp(-i tau (c alpha.(k - q Abar) + m c^2 beta)) of PAPER.md:203-232
+ * (eq. 27-33) and 240-242 (eq. 35) for Dirac.  Units: atomic units, hbar = 1
+ * (PAPER.md:323).
+ *
+ * Conventions:
+ *   grid      r_j = (j - n/2) dx per axis, half open, periodic (G14, G18)
+ *   momenta   k_j = 2 pi j/(n dx), j < n/2;  2 pi (j-n)/(n dx), j >= n/2 (Nyquist negative)
+ *   DFT       forward = exp(-i k.r), unnormalised; inverse carries 1/N (eq. 12)
+ *   layout    psi[ncomp][n0][n1][n2], C order, last axis contiguous, interleaved (re, im),
+ *             float2 (SSO_C64) or double2 (SSO_C128)
+ *   Dirac     ncomp = 4: Dirac representation, PAPER.md:127-129 (eq. 16);
+ *             ncomp = 2: alpha_1 = sigma_x, alpha_2 = sigma_y, beta = sigma_z
+ *             (eq. 17 and the {1,4} block of eq. 16, reading G7)
+ *   fields    time integrals over a step are supplied by the caller as step AVERAGES
+ *             (reading G12); both potential half steps of step n use the same average (G13)
+ *
+ * All device work is enqueued on the caller's CUDA stream (a cudaStream_t passed
+ * as void*; NULL = the legacy default stream) and is asynchronous, except
+ * sso_norm, sso_step_host and the table uploads of sso_set_*, which synchronise
+ * that stream.  There is no CPU fallback: every entry point that needs the GPU
+ * fails with SSO_ERR_CUDA when no device is usable.
+ *
+ * Error behaviour: every function returns an int status (0 = SSO_OK); nothing is
+ * thrown across the ABI.  sso_last_error(plan) returns a plan-owned, NUL-terminated
+ * description of the most recent failure on that plan (or, for plan == NULL, of the
+ * most recent failed sso_plan_create on this thread).
+ */
+#ifndef SSO_H_
+#define SSO_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SSO_OK 0
+#define SSO_ERR_INVALID 1     /* bad argument (NULL, range, alignment, non-finite)          */
+#define SSO_ERR_UNSUPPORTED 2 /* valid request this build does not implement                */
+#define SSO_ERR_ALLOC 3       /* host or device allocation failed                           */
+#define SSO_ERR_CUDA 4        /* CUDA runtime error, or no device                           */
+#define SSO_ERR_STATE 5       /* call sequence error (e.g. field table too short for nsteps) */
+
+#define SSO_C64 0  /* complex64:  float2  */
+#define SSO_C128 1 /* complex128: double2 */
+
+#define SSO_FIELD_NONE 0
+#define SSO_FIELD_E 1 /* length gauge: adds r . Ebar_n to the potential energy (eq. 11) */
+#define SSO_FIELD_A 2 /* velocity gauge, homogeneous A(t): pi = k - q Abar_n in the kinetic factor
+                         (eq. 13; for Dirac reading G16)                              */
+
+/* options for sso_set_option */
+#define SSO_OPT_LINES_PER_TILE_CONTIG 1  /* lines per CTA in contiguous-axis passes (0 = auto)   */
+#define SSO_OPT_LINES_PER_TILE_STRIDED 2 /* adjacent lines per CTA in strided-axis passes (0=auto) */
+#define SSO_OPT_POTENTIAL_PHASE 3        /* 0 = complex phase table exp(-i V tau/2) (default),
+                                            1 = real angle table + in-kernel sincos polynomial   */
+
+#define SSO_MIN_AXIS 16   /* smallest supported axis length                       */
+#define SSO_MAX_AXIS 4096 /* largest supported axis length (one CTA holds a line) */
+
+typedef struct sso_plan sso_plan; /* opaque; owned by the library */
+
+/*
+ * Create a plan for a lattice of `ndim` (1..3) axes with sizes[a] points (powers
+ * of two in [SSO_MIN_AXIS, SSO_MAX_AXIS]) and spacings dx[a] > 0, time step dt
+ * (finite, may be negative: the Strang step is symmetric, so -dt undoes +dt),
+ * ncomp = 1 (Schroedinger), 2 (Dirac, ndim 1 or 2) or 4 (Dirac, ndim 1..3).
+ * sizes and dx are host arrays, read during the call only.  Builds the radix
+ * schedule, twiddle tables and k grids.  Defaults: V = 0, no
+ * field, mass 1, c 137.036, charge -1 (electron), time index 0.
+ * On failure *out is set to NULL.
+ */
+int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double *dx, double dt,
+                    int ncomp, int precision);
+
+/* Particle constants m, c, q (eq. 9, 117 eq. 14).  mass > 0, c > 0, all finite. */
+int sso_set_constants(sso_plan *plan, double mass, double c, double charge);
+
+/*
+ * Real potential ENERGY q phi(r) on the lattice, double[n0][n1][n2] in C order
+ * (host pointer if on_device == 0, device pointer otherwise); NULL means V = 0.
+ * The array is consumed during the call (the plan keeps its own phase table
+ * exp(-i V tau/2), eq. 11 with delta = 1/2); the caller keeps
+ * ownership.  Synchronises `stream`.
+ */
+int sso_set_potential(sso_plan *plan, const double *V, int on_device, void *stream);
+
+/*
+ * Homogeneous, time-dependent field.  step_avg is a HOST array
+ * double[nvals][ndim]: row n holds the average over [n dt, (n+1) dt] of E(t)
+ * (SSO_FIELD_E) or A(t) (SSO_FIELD_A).  Copied; kind SSO_FIELD_NONE ignores the
+ * other arguments.  Stepping past row nvals-1 fails with SSO_ERR_STATE.
+ */
+int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nvals);
+
+/* Step counter n used to index step_avg (t_n = n dt, reading G21); sso_step advances it. */
+int sso_set_time_index(sso_plan *plan, int64_t n);
+int sso_get_time_index(const sso_plan *plan, int64_t *n);
+
+/*
+ * Advance psi in place by nsteps >= 0 steps.  psi is a DEVICE pointer to
+ * ncomp * prod(sizes) complex numbers in the plan's precision, 16-byte aligned;
+ * the caller owns it.  Asynchronous on `stream`; only kernels are enqueued (the
+ * call can be captured into a CUDA graph).  Consecutive potential half steps
+ * inside one call are merged into one phase (identical up to rounding).
+ */
+int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream);
+
+/*
+ * Same, for a HOST buffer: copies psi to a plan-owned device buffer, steps,
+ * copies back and synchronises (the paper's protocol: one upload before the
+ * first step, one download after the last).
+ */
+int sso_step_host(sso_plan *plan, void *psi_host, int64_t nsteps);
+
+/* *out_host = sum_c sum_r |psi_c(r)|^2 prod(dx), accumulated in double.  Synchronises `stream`. */
+int sso_norm(sso_plan *plan, const void *psi, double *out_host, void *stream);
+
+/* Tuning knobs (SSO_OPT_*); invalid values give SSO_ERR_INVALID. */
+int sso_set_option(sso_plan *plan, int option, int64_t value);
+
+/*
+ * Number of kernel launches sso_step(nsteps) enqueues for this plan in its
+ * current state (for launch accounting in benchmarks).
+ */
+int sso_launch_count(const sso_plan *plan, int64_t nsteps, int64_t *count);
+
+/* Frees every table; NULL is a no-op returning SSO_OK. */
+int sso_destroy(sso_plan *plan);
+
+const char *sso_last_error(const sso_plan *plan);
+
+/* Library version string, e.g. "sso 0.1 (sm_100a)". */
+const char *sso_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SSO_H_ */

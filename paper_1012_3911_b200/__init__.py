@@ -1,0 +1,168 @@
+"""paper_1012_3911_b200 -- Python binding of libsso.so, the B200-native Fourier split-operator library.
+
+Argument marshalling only: every step of the path (potential phases, FFTs, kinetic factors, norm)
+runs in the CUDA kernels behind the C ABI declared in ``include/sso.h``.  PyTorch is used by callers
+for device memory and streams; this module needs neither torch nor numpy to load.  There is no CPU
+fallback: if the shared library is missing the import of :func:`lib` fails loudly.
+
+The operation is one Fourier split-operator step (eq. 7, 76 eq. 8) -- see
+``include/sso.h`` for the conventions.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+from typing import Optional, Sequence
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libsso.so"
+
+OK, ERR_INVALID, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_STATE = 0, 1, 2, 3, 4, 5
+C64, C128 = 0, 1
+FIELD_NONE, FIELD_E, FIELD_A = 0, 1, 2
+OPT_LINES_PER_TILE_CONTIG, OPT_LINES_PER_TILE_STRIDED, OPT_POTENTIAL_PHASE = 1, 2, 3
+
+# every symbol include/sso.h declares
+SYMBOLS = (
+    "sso_plan_create", "sso_set_constants", "sso_set_potential", "sso_set_field", "sso_set_time_index",
+    "sso_get_time_index", "sso_step", "sso_step_host", "sso_norm", "sso_set_option", "sso_launch_count",
+    "sso_destroy", "sso_last_error", "sso_version",
+)
+
+
+class SsoError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"sso error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libsso.so (built in-tree by ``paper_1012_3911_b200.build``); raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise ImportError(f"{LIB_PATH} not found: run `python -m paper_1012_3911_b200.build` (there is no CPU fallback)")
+        L = ctypes.CDLL(str(LIB_PATH))
+        vp, i64, dbl, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
+        L.sso_plan_create.argtypes = [ctypes.POINTER(vp), ci, ctypes.POINTER(i64), ctypes.POINTER(dbl), dbl, ci, ci]
+        L.sso_set_constants.argtypes = [vp, dbl, dbl, dbl]
+        L.sso_set_potential.argtypes = [vp, vp, ci, vp]
+        L.sso_set_field.argtypes = [vp, ci, vp, i64]
+        L.sso_set_time_index.argtypes = [vp, i64]
+        L.sso_get_time_index.argtypes = [vp, ctypes.POINTER(i64)]
+        L.sso_step.argtypes = [vp, vp, i64, vp]
+        L.sso_step_host.argtypes = [vp, vp, i64]
+        L.sso_norm.argtypes = [vp, vp, ctypes.POINTER(dbl), vp]
+        L.sso_set_option.argtypes = [vp, ci, i64]
+        L.sso_launch_count.argtypes = [vp, i64, ctypes.POINTER(i64)]
+        L.sso_destroy.argtypes = [vp]
+        L.sso_last_error.argtypes = [vp]
+        L.sso_last_error.restype = ctypes.c_char_p
+        L.sso_version.restype = ctypes.c_char_p
+        for name in SYMBOLS:
+            if name not in ("sso_last_error", "sso_version"):
+                getattr(L, name).restype = ci
+        _lib = L
+    return _lib
+
+
+def version() -> str:
+    return lib().sso_version().decode()
+
+
+def _ptr(x) -> Optional[int]:
+    """Address of a torch tensor / numpy array / raw int; None stays NULL."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):
+        return x.ctypes.data
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _stream(s) -> Optional[int]:
+    if s is None:
+        return None
+    if isinstance(s, int):
+        return s or None
+    return s.cuda_stream  # torch.cuda.Stream
+
+
+class Plan:
+    """Thin owner of an ``sso_plan*``; method names follow the C ABI (sso_<name>)."""
+
+    def __init__(self, sizes: Sequence[int], dx: Sequence[float], dt: float, ncomp: int = 1, precision: int = C128):
+        L = lib()
+        nd = len(sizes)
+        self._h = ctypes.c_void_p()
+        szs = (ctypes.c_int64 * max(nd, 1))(*[int(s) for s in sizes])
+        dxs = (ctypes.c_double * max(nd, 1))(*[float(d) for d in dx])
+        rc = L.sso_plan_create(ctypes.byref(self._h), nd, szs, dxs, float(dt), int(ncomp), int(precision))
+        if rc != OK:
+            raise SsoError(rc, L.sso_last_error(None).decode())
+        self.sizes, self.ncomp, self.precision = tuple(int(s) for s in sizes), int(ncomp), int(precision)
+
+    def _ck(self, rc: int) -> None:
+        if rc != OK:
+            raise SsoError(rc, lib().sso_last_error(self._h).decode())
+
+    def set_constants(self, mass: float, c: float, charge: float) -> None:
+        self._ck(lib().sso_set_constants(self._h, mass, c, charge))
+
+    def set_potential(self, V, on_device: bool = False, stream=None) -> None:
+        """V: float64 array of shape sizes (numpy on host, or a torch CUDA tensor with on_device=True); None = 0."""
+        self._ck(lib().sso_set_potential(self._h, _ptr(V), int(bool(on_device)), _stream(stream)))
+
+    def set_field(self, kind: int, step_avg=None) -> None:
+        """step_avg: contiguous float64 host array [nvals][ndim]."""
+        if kind == FIELD_NONE or step_avg is None:
+            self._ck(lib().sso_set_field(self._h, int(kind), None, 0))
+            return
+        nvals = step_avg.shape[0]
+        self._ck(lib().sso_set_field(self._h, int(kind), _ptr(step_avg), int(nvals)))
+
+    def set_time_index(self, n: int) -> None:
+        self._ck(lib().sso_set_time_index(self._h, int(n)))
+
+    def get_time_index(self) -> int:
+        n = ctypes.c_int64()
+        self._ck(lib().sso_get_time_index(self._h, ctypes.byref(n)))
+        return n.value
+
+    def set_option(self, option: int, value: int) -> None:
+        self._ck(lib().sso_set_option(self._h, int(option), int(value)))
+
+    def step(self, psi, nsteps: int, stream=None) -> None:
+        """psi: device buffer (torch CUDA tensor, complex64/complex128, shape (ncomp, *sizes)); in place, asynchronous."""
+        self._ck(lib().sso_step(self._h, _ptr(psi), int(nsteps), _stream(stream)))
+
+    def step_host(self, psi_host, nsteps: int) -> None:
+        """psi_host: host buffer (numpy array or pinned torch tensor); copied up, stepped, copied back."""
+        self._ck(lib().sso_step_host(self._h, _ptr(psi_host), int(nsteps)))
+
+    def norm(self, psi, stream=None) -> float:
+        out = ctypes.c_double()
+        self._ck(lib().sso_norm(self._h, _ptr(psi), ctypes.byref(out), _stream(stream)))
+        return out.value
+
+    def launch_count(self, nsteps: int) -> int:
+        n = ctypes.c_int64()
+        self._ck(lib().sso_launch_count(self._h, int(nsteps), ctypes.byref(n)))
+        return n.value
+
+    def destroy(self) -> None:
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().sso_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

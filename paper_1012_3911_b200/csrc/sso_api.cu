@@ -1,0 +1,786 @@
+// sso_api.cu -- the C ABI of include/sso.h: plan builder (radix schedule, twiddles, k grids,
+// phase tables), the per-step pass schedule, and the small auxiliary kernels (table builders,
+// norm reduction).  The pass kernel itself is in sso_pass.cuh.
+//
+// Pass schedule: 1D FFTs along different axes commute and the trailing
+// potential half step of step n merges with the leading one of step n+1 (eq. 7
+// applied twice), so a steady-state step costs
+//   1D: 0 round trips of psi through HBM (one persistent CTA keeps the line in registers),
+//   2D: 2 passes   [F_1^-1 V F_1]  [F_0 K F_0^-1]
+//   3D: 4 passes   [F_2^-1 V F_2]  [F_1]  [F_0 K F_0^-1]  [F_1^-1]
+// plus one opening [F_last V/2] and one closing [V/2 F_last^-1] pass per sso_step call.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/sso.h"
+#include "sso_dispatch.h"
+
+namespace sso {
+
+// ---------------------------------------------------------------------------------------------
+// auxiliary kernels
+// ---------------------------------------------------------------------------------------------
+
+template <typename T> struct Cx2;
+template <> struct Cx2<float> { using type = float2; };
+template <> struct Cx2<double> { using type = double2; };
+
+// potential phase table: out[line*N + slot] = exp(-i V[line*N + nat(slot)] tau/2)  (eq. 11, delta = 1/2)
+// or, for the angle representation, the angle -V tau/2 reduced to [-pi, pi).
+template <typename T>
+__global__ void build_vtab_kernel(const double *__restrict__ V, void *__restrict__ out, long long total, int N,
+                                  const int *__restrict__ slot_nat, double half_dt, int vrep) {
+    using C = typename Cx2<T>::type;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const long long line = i / N;
+        const int slot = (int)(i % N);
+        const int nat = slot_nat ? slot_nat[slot] : slot;
+        const double v = V ? V[line * N + nat] : 0.0;
+        const double ang = -v * half_dt;
+        if (vrep == VREP_TABLE) {
+            double s, c;
+            sincos(ang, &s, &c);
+            C h;
+            h.x = (T)c;
+            h.y = (T)s;
+            reinterpret_cast<C *>(out)[i] = h;
+        } else {
+            const double twopi = 6.283185307179586476925286766559;
+            reinterpret_cast<double *>(out)[i] = ang - twopi * rint(ang / twopi);
+        }
+    }
+}
+
+// Schroedinger kinetic phase of one axis: out[i] = scale * exp(-i tau (k[i] - shift)^2 / (2 m))   (eq. 13)
+template <typename T>
+__global__ void build_kphase_kernel(const double *__restrict__ kv, void *__restrict__ out, int n, double tau, double mass,
+                                    const double *__restrict__ step_avg, long long row, int ndim, int axis, double charge, double scale) {
+    using C = typename Cx2<T>::type;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double shift = step_avg ? charge * step_avg[row * ndim + axis] : 0.0;
+    const double p = kv[i] - shift;
+    const double ang = -tau * p * p / (2.0 * mass);
+    double s, c;
+    sincos(ang, &s, &c);
+    C h;
+    h.x = (T)(c * scale);
+    h.y = (T)(s * scale);
+    reinterpret_cast<C *>(out)[i] = h;
+}
+
+// phase of a homogeneous E field along the line axis in the permuted layout:
+// out[slot] = exp(-i (tau/2) (E_na + [full] E_nb)[axis] r(nat(slot)))
+template <typename T>
+__global__ void build_ephase_kernel(void *__restrict__ out, int n, const int *__restrict__ slot_nat, double dx, double half_dt,
+                                    const double *__restrict__ step_avg, long long na, long long nb, int full, int ndim, int axis) {
+    using C = typename Cx2<T>::type;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double e = step_avg[na * ndim + axis];
+    if (full) e += step_avg[nb * ndim + axis];
+    const double r = ((double)slot_nat[i] - (double)(n / 2)) * dx;
+    double s, c;
+    sincos(-e * half_dt * r, &s, &c);
+    C h;
+    h.x = (T)c;
+    h.y = (T)s;
+    reinterpret_cast<C *>(out)[i] = h;
+}
+
+// norm: partial sums of |psi|^2 in double, warp-shuffle tree, fixed order (deterministic)
+template <typename T>
+__global__ void norm_partial_kernel(const void *__restrict__ psi, long long count, double *__restrict__ partial) {
+    using C = typename Cx2<T>::type;
+    const C *p = reinterpret_cast<const C *>(psi);
+    double acc = 0.0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < count; i += (long long)gridDim.x * blockDim.x) {
+        const C v = p[i];
+        acc += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
+    }
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+    __shared__ double wsum[32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) wsum[w] = acc;
+    __syncthreads();
+    if (w == 0) {
+        acc = lane < (int)(blockDim.x >> 5) ? wsum[lane] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+        if (lane == 0) partial[blockIdx.x] = acc;
+    }
+}
+__global__ void norm_final_kernel(const double *__restrict__ partial, int n, double vol, double *__restrict__ out) {
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < n; i += 32) acc += partial[i];
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+    if (threadIdx.x == 0) *out = acc * vol;
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+
+static LaunchFn find_launch(int precision, int N, int strided, int pw, int sign) {
+    switch (N) {
+#define SSO_CASE(NN) \
+    case NN:         \
+        return precision == SSO_C64 ? sso_lookup_f32_##NN(strided, pw, sign) : sso_lookup_f64_##NN(strided, pw, sign);
+        SSO_FOR_EACH_N(SSO_CASE)
+#undef SSO_CASE
+    }
+    return nullptr;
+}
+
+// the radix schedule of sso_pass.cuh's Sched<N>, at run time
+struct HostSched {
+    int m;
+    int lr[8];
+    explicit HostSched(int N) {
+        int LOG = 0;
+        while ((1 << LOG) < N) ++LOG;
+        const int REM = LOG - 4;
+        m = 1 + (REM + 3) / 4;
+        for (int i = 0; i < m; ++i) lr[i] = (i == m - 1) ? 4 : (i == 0 ? REM - 4 * (m - 2) : 4);
+    }
+};
+
+// frequency index held at network position p after the DIF stages: p = sum_i k_i N_i  ->  k_1 + R_1 k_2 + R_1 R_2 k_3 + ...
+static int freq_of_pos(int N, int p) {
+    HostSched s(N);
+    int Ni = N, w = 1, f = 0;
+    for (int i = 0; i < s.m; ++i) {
+        const int R = 1 << s.lr[i];
+        Ni /= R;
+        const int k = (p / Ni) % R;
+        f += k * w;
+        w *= R;
+    }
+    return f;
+}
+
+struct Axis {
+    int n = 0;
+    double dx = 0.0;
+    std::vector<double> k_nat;     // k_j in DFT order (Nyquist negative, reading G14)
+    std::vector<int> pos_freq;     // network position -> frequency index
+    std::vector<int> slot_nat;     // permuted-layout slot (q U + B') -> natural index
+    void *tw = nullptr;            // device complex[n]
+    int *d_revB = nullptr;         // device int[n/16]
+    int *d_revBinv = nullptr;      // device int[n/16]
+    int *d_slot_nat = nullptr;     // device int[n]
+    double *d_kv = nullptr;        // device double[n]: k in the layout this axis uses in the kinetic pass
+    void *d_kph = nullptr;         // device complex[n]: Schroedinger phase table in the same layout
+    void *d_ephase = nullptr;      // device complex[n]: E-field phase along this axis (last axis only)
+};
+
+}  // namespace sso
+
+using namespace sso;
+
+struct sso_plan {
+    int ndim = 0, ncomp = 1, precision = SSO_C128;
+    Axis ax[3];
+    long long npts = 1;
+    double dt = 0.0;
+    double mass = 1.0, clight = 137.036, charge = -1.0;
+    int field_kind = SSO_FIELD_NONE;
+    std::vector<double> h_avg;  // [nvals][ndim]
+    long long nvals = 0;
+    double *d_avg = nullptr;
+    bool e_along_last = false;  // some row has a nonzero E component along the last axis
+    long long tindex = 0;
+    void *d_vtab = nullptr;
+    int vrep = VREP_TABLE;
+    bool kph_valid = false;
+    int opt_tl_contig = 0, opt_tl_strided = 0;
+    double *d_partial = nullptr, *d_norm = nullptr;
+    void *d_hostbuf = nullptr;
+    std::string err;
+    size_t esize() const { return precision == SSO_C64 ? 8 : 16; }
+};
+
+static thread_local std::string g_create_err;
+static const int NORM_BLOCKS = 592;
+
+static int fail(sso_plan *p, int code, const std::string &msg) {
+    if (p) p->err = msg;
+    else g_create_err = msg;
+    return code;
+}
+static int cuda_fail(sso_plan *p, cudaError_t e, const char *what) {
+    return fail(p, SSO_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                                  \
+    do {                                                          \
+        cudaError_t e_ = (call);                                  \
+        if (e_ != cudaSuccess) return cuda_fail(plan, e_, #call); \
+    } while (0)
+
+template <typename V> static cudaError_t upload(void **dst, const std::vector<V> &src) {
+    cudaError_t e = cudaMalloc(dst, src.size() * sizeof(V));
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(*dst, src.data(), src.size() * sizeof(V), cudaMemcpyHostToDevice);
+}
+
+static bool is_pow2(long long v) { return v > 0 && (v & (v - 1)) == 0; }
+
+// which layout the kinetic tables of axis a use: axis 0 is the kinetic-sandwich axis (permuted slots),
+// the middle axis of a 3D lattice is stored in network order, the last axis of a >=2D lattice is natural
+static void kinetic_layout(const sso_plan *p, int a, std::vector<double> &kv) {
+    const Axis &A = p->ax[a];
+    kv.resize(A.n);
+    if (a == 0) {
+        for (int s = 0; s < A.n; ++s) kv[s] = A.k_nat[A.slot_nat[s]];
+    } else if (a == 1 && p->ndim == 3) {
+        for (int q = 0; q < A.n; ++q) kv[q] = A.k_nat[A.pos_freq[q]];
+    } else {
+        kv = A.k_nat;
+    }
+}
+
+extern "C" {
+
+const char *sso_version(void) { return "sso 0.1 (sm_100a)"; }
+
+const char *sso_last_error(const sso_plan *plan) { return plan ? plan->err.c_str() : g_create_err.c_str(); }
+
+int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double *dx, double dt, int ncomp, int precision) {
+    sso_plan *plan = nullptr;  // for CK / fail before the plan exists
+    if (!out) return fail(nullptr, SSO_ERR_INVALID, "out is NULL");
+    *out = nullptr;
+    if (!sizes || !dx) return fail(nullptr, SSO_ERR_INVALID, "sizes or dx is NULL");
+    if (ndim < 1 || ndim > 3) return fail(nullptr, SSO_ERR_INVALID, "ndim must be 1, 2 or 3");
+    if (precision != SSO_C64 && precision != SSO_C128) return fail(nullptr, SSO_ERR_INVALID, "precision must be SSO_C64 or SSO_C128");
+    if (ncomp != 1 && ncomp != 2 && ncomp != 4) return fail(nullptr, SSO_ERR_INVALID, "ncomp must be 1, 2 or 4");
+    if (ncomp == 2 && ndim == 3) return fail(nullptr, SSO_ERR_INVALID, "a 2-component Dirac spinor exists in 1 and 2 dimensions only");
+    if (!isfinite(dt)) return fail(nullptr, SSO_ERR_INVALID, "dt must be finite");
+    for (int a = 0; a < ndim; ++a) {
+        if (!(dx[a] > 0.0) || !isfinite(dx[a])) return fail(nullptr, SSO_ERR_INVALID, "dx must be positive and finite");
+        if (!is_pow2(sizes[a])) return fail(nullptr, SSO_ERR_INVALID, "sizes must be powers of two");
+        if (sizes[a] < SSO_MIN_AXIS || sizes[a] > SSO_MAX_AXIS)
+            return fail(nullptr, SSO_ERR_UNSUPPORTED, "axis length outside [16, 4096]");
+    }
+    if (ncomp > 1 && (long long)ncomp * (sizes[0] / 16) > 512)
+        return fail(nullptr, SSO_ERR_UNSUPPORTED, "Dirac plans need ncomp * sizes[0] <= 8192 (all components of a line share one CTA)");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, SSO_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    }
+    plan = new (std::nothrow) sso_plan();
+    if (!plan) return fail(nullptr, SSO_ERR_ALLOC, "out of host memory");
+    plan->ndim = ndim;
+    plan->ncomp = ncomp;
+    plan->precision = precision;
+    plan->dt = dt;
+    const double PI = 3.14159265358979323846264338327950288;
+    for (int a = 0; a < ndim; ++a) {
+        Axis &A = plan->ax[a];
+        A.n = (int)sizes[a];
+        A.dx = dx[a];
+        plan->npts *= A.n;
+        const int n = A.n, U = n / 16;
+        A.k_nat.resize(n);
+        for (int j = 0; j < n; ++j) {
+            const int jj = j < n / 2 ? j : j - n;
+            A.k_nat[j] = 2.0 * PI * (double)jj / ((double)n * A.dx);
+        }
+        A.pos_freq.resize(n);
+        A.slot_nat.resize(n);
+        std::vector<int> revB(U), revBinv(U);
+        for (int p = 0; p < n; ++p) {
+            const int f = freq_of_pos(n, p);
+            A.pos_freq[p] = f;
+            A.slot_nat[(p % 16) * U + p / 16] = f;
+            if (p % 16 == 0) {
+                revB[p / 16] = f;
+                revBinv[f] = p / 16;
+            }
+        }
+        // twiddles exp(-2 pi i t/n), evaluated in long double and rounded once to the plan's precision
+        cudaError_t e;
+        if (precision == SSO_C128) {
+            std::vector<double2> tw(n);
+            for (int t = 0; t < n; ++t) {
+                const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)t / (long double)n;
+                tw[t].x = (double)cosl(ang);
+                tw[t].y = (double)sinl(ang);
+            }
+            e = upload(&A.tw, tw);
+        } else {
+            std::vector<float2> tw(n);
+            for (int t = 0; t < n; ++t) {
+                const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)t / (long double)n;
+                tw[t].x = (float)cosl(ang);
+                tw[t].y = (float)sinl(ang);
+            }
+            e = upload(&A.tw, tw);
+        }
+        if (e == cudaSuccess) e = upload((void **)&A.d_revB, revB);
+        if (e == cudaSuccess) e = upload((void **)&A.d_revBinv, revBinv);
+        if (e == cudaSuccess) e = upload((void **)&A.d_slot_nat, A.slot_nat);
+        std::vector<double> kv;
+        kinetic_layout(plan, a, kv);
+        if (e == cudaSuccess) e = upload((void **)&A.d_kv, kv);
+        if (e == cudaSuccess) e = cudaMalloc(&A.d_kph, (size_t)n * plan->esize());
+        if (e == cudaSuccess) e = cudaMalloc(&A.d_ephase, (size_t)n * plan->esize());
+        if (e != cudaSuccess) {
+            int rc = cuda_fail(nullptr, e, "plan tables");
+            sso_destroy(plan);
+            return rc;
+        }
+    }
+    cudaError_t e = cudaMalloc((void **)&plan->d_partial, sizeof(double) * NORM_BLOCKS);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&plan->d_norm, sizeof(double));
+    if (e != cudaSuccess) {
+        int rc = cuda_fail(nullptr, e, "plan buffers");
+        sso_destroy(plan);
+        return rc;
+    }
+    int rc = sso_set_potential(plan, nullptr, 0, nullptr);
+    if (rc != SSO_OK) {
+        g_create_err = plan->err;
+        sso_destroy(plan);
+        return rc;
+    }
+    *out = plan;
+    return SSO_OK;
+}
+
+int sso_destroy(sso_plan *plan) {
+    if (!plan) return SSO_OK;
+    for (int a = 0; a < 3; ++a) {
+        Axis &A = plan->ax[a];
+        cudaFree(A.tw);
+        cudaFree(A.d_revB);
+        cudaFree(A.d_revBinv);
+        cudaFree(A.d_slot_nat);
+        cudaFree(A.d_kv);
+        cudaFree(A.d_kph);
+        cudaFree(A.d_ephase);
+    }
+    cudaFree(plan->d_avg);
+    cudaFree(plan->d_vtab);
+    cudaFree(plan->d_partial);
+    cudaFree(plan->d_norm);
+    cudaFree(plan->d_hostbuf);
+    delete plan;
+    return SSO_OK;
+}
+
+int sso_set_constants(sso_plan *plan, double mass, double c, double charge) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (!(mass > 0.0) || !(c > 0.0) || !isfinite(mass) || !isfinite(c) || !isfinite(charge))
+        return fail(plan, SSO_ERR_INVALID, "mass and c must be positive, all constants finite");
+    plan->mass = mass;
+    plan->clight = c;
+    plan->charge = charge;
+    plan->kph_valid = false;
+    return SSO_OK;
+}
+
+int sso_set_potential(sso_plan *plan, const double *V, int on_device, void *stream) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long total = plan->npts;
+    const double *dV = nullptr;
+    double *tmp = nullptr;
+    if (V && !on_device) {
+        CK(cudaMalloc((void **)&tmp, sizeof(double) * total));
+        cudaError_t e = cudaMemcpyAsync(tmp, V, sizeof(double) * total, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) {
+            cudaFree(tmp);
+            return cuda_fail(plan, e, "upload of V");
+        }
+        dV = tmp;
+    } else {
+        dV = V;
+    }
+    const size_t entry = plan->vrep == VREP_TABLE ? plan->esize() : sizeof(double);
+    cudaFree(plan->d_vtab);
+    plan->d_vtab = nullptr;
+    cudaError_t e = cudaMalloc(&plan->d_vtab, entry * total);
+    if (e != cudaSuccess) {
+        cudaFree(tmp);
+        return fail(plan, SSO_ERR_ALLOC, std::string("potential table: ") + cudaGetErrorString(e));
+    }
+    const Axis &L = plan->ax[plan->ndim - 1];
+    const int *slot_nat = plan->ndim >= 2 ? L.d_slot_nat : nullptr;  // 1D keeps the natural order
+    const int blocks = (int)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
+    if (plan->precision == SSO_C128)
+        build_vtab_kernel<double><<<blocks, 256, 0, st>>>(dV, plan->d_vtab, total, L.n, slot_nat, 0.5 * plan->dt, plan->vrep);
+    else
+        build_vtab_kernel<float><<<blocks, 256, 0, st>>>(dV, plan->d_vtab, total, L.n, slot_nat, 0.5 * plan->dt, plan->vrep);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(tmp);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "potential table kernel");
+    return SSO_OK;
+}
+
+int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nvals) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (kind != SSO_FIELD_NONE && kind != SSO_FIELD_E && kind != SSO_FIELD_A) return fail(plan, SSO_ERR_INVALID, "unknown field kind");
+    if (kind == SSO_FIELD_NONE) {
+        plan->field_kind = kind;
+        plan->h_avg.clear();
+        plan->nvals = 0;
+        cudaFree(plan->d_avg);
+        plan->d_avg = nullptr;
+        plan->e_along_last = false;
+        plan->kph_valid = false;
+        return SSO_OK;
+    }
+    if (!step_avg || nvals <= 0) return fail(plan, SSO_ERR_INVALID, "step_avg is NULL or nvals <= 0");
+    const size_t cnt = (size_t)nvals * plan->ndim;
+    for (size_t i = 0; i < cnt; ++i)
+        if (!isfinite(step_avg[i])) return fail(plan, SSO_ERR_INVALID, "step_avg holds a non-finite value");
+    double *d = nullptr;
+    CK(cudaMalloc((void **)&d, sizeof(double) * cnt));
+    cudaError_t e = cudaMemcpy(d, step_avg, sizeof(double) * cnt, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        cudaFree(d);
+        return cuda_fail(plan, e, "upload of step_avg");
+    }
+    cudaFree(plan->d_avg);
+    plan->d_avg = d;
+    plan->h_avg.assign(step_avg, step_avg + cnt);
+    plan->nvals = nvals;
+    plan->field_kind = kind;
+    plan->e_along_last = false;
+    if (kind == SSO_FIELD_E)
+        for (int64_t n = 0; n < nvals; ++n)
+            if (step_avg[n * plan->ndim + plan->ndim - 1] != 0.0) plan->e_along_last = true;
+    plan->kph_valid = false;
+    return SSO_OK;
+}
+
+int sso_set_time_index(sso_plan *plan, int64_t n) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (n < 0) return fail(plan, SSO_ERR_INVALID, "time index must be >= 0");
+    plan->tindex = n;
+    return SSO_OK;
+}
+
+int sso_get_time_index(const sso_plan *plan, int64_t *n) {
+    if (!plan || !n) return SSO_ERR_INVALID;
+    *n = plan->tindex;
+    return SSO_OK;
+}
+
+int sso_set_option(sso_plan *plan, int option, int64_t value) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    switch (option) {
+        case SSO_OPT_LINES_PER_TILE_CONTIG:
+        case SSO_OPT_LINES_PER_TILE_STRIDED:
+            if (value < 0 || value > 512 || (value > 0 && !is_pow2(value))) return fail(plan, SSO_ERR_INVALID, "lines per tile must be 0 or a power of two <= 512");
+            (option == SSO_OPT_LINES_PER_TILE_CONTIG ? plan->opt_tl_contig : plan->opt_tl_strided) = (int)value;
+            return SSO_OK;
+        case SSO_OPT_POTENTIAL_PHASE:
+            if (value != VREP_TABLE && value != VREP_ANGLE) return fail(plan, SSO_ERR_INVALID, "potential phase mode must be 0 or 1");
+            if ((int)value != plan->vrep) {
+                plan->vrep = (int)value;
+                // the table is rebuilt by the next sso_set_potential; until then V = 0
+                return sso_set_potential(plan, nullptr, 0, nullptr);
+            }
+            return SSO_OK;
+    }
+    return fail(plan, SSO_ERR_INVALID, "unknown option");
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// pass construction
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+struct Geometry {
+    int axis;          // lattice axis of the lines
+    bool strided;
+    long long inner;   // element stride along the line
+    long long lines;   // lines per component
+    int rest1;
+    int oaxA, oaxB;
+};
+
+Geometry geometry(const sso_plan *p, int axis) {
+    Geometry g{};
+    g.axis = axis;
+    const int nd = p->ndim;
+    g.inner = 1;
+    for (int a = axis + 1; a < nd; ++a) g.inner *= p->ax[a].n;
+    g.strided = g.inner > 1;
+    g.lines = p->npts / p->ax[axis].n;
+    g.oaxA = g.oaxB = -1;
+    g.rest1 = 1;
+    int others[2], no = 0;
+    for (int a = 0; a < nd; ++a)
+        if (a != axis) others[no++] = a;
+    if (no == 1) {
+        g.oaxB = others[0];
+        g.rest1 = p->ax[others[0]].n;
+    } else if (no == 2) {
+        g.oaxA = others[0];
+        g.oaxB = others[1];
+        g.rest1 = p->ax[others[1]].n;
+    }
+    return g;
+}
+
+// lines per component per CTA
+int choose_tl(const sso_plan *p, const Geometry &g, int cc) {
+    const int U = p->ax[g.axis].n / 16;
+    const int esz = (int)p->esize();
+    long long tl;
+    if (!g.strided) {
+        tl = p->opt_tl_contig > 0 ? p->opt_tl_contig : 256 / (cc * U);
+        if (tl < 1) tl = 1;
+        if (tl > g.lines) tl = g.lines;
+    } else {
+        const int tlmin = 32 / esz < 1 ? 1 : 32 / esz;  // at least one 32-byte sector per line element
+        tl = p->opt_tl_strided > 0 ? p->opt_tl_strided : 256 / (cc * U);
+        if (p->opt_tl_strided == 0 && tl < tlmin) tl = tlmin;
+        if (tl > g.inner) tl = g.inner;
+    }
+    while (tl > 1 && (long long)cc * tl * U > 512) tl /= 2;
+    return (int)tl;
+}
+
+struct PassSpec {
+    int axis;
+    int pw;        // PW_*
+    int sign;      // sign of the DIF transform
+    int do_dif, do_dit, unpermute, mid_on, pre_v, post_v;
+    int v_mid_full;
+    int nrep;
+    long long n;   // step index
+};
+
+int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
+    const Geometry g = geometry(plan, s.axis);
+    const Axis &A = plan->ax[s.axis];
+    const int cc = s.pw == PW_KD2 ? 2 : (s.pw == PW_KD4 ? 4 : 1);
+    const int U = A.n / 16;
+    const int TL = choose_tl(plan, g, cc);
+    const int esz = (int)plan->esize();
+    PassArgs a{};
+    a.psi = psi;
+    a.tw = A.tw;
+    a.revB = A.d_revB;
+    a.revBinv = A.d_revBinv;
+    a.comp_stride = plan->npts;
+    a.inner = g.inner;
+    a.ncomp = plan->ncomp;
+    a.TL = TL;
+    int pitch = A.n + A.n / 16;
+    if (g.strided) {
+        const int G = 128 / esz;
+        pitch += (G / TL > 1 ? G / TL : 1);
+    }
+    a.pitch = pitch;
+    a.rest1 = g.rest1;
+    a.oaxA = g.oaxA;
+    a.oaxB = g.oaxB;
+    a.do_dif = s.do_dif;
+    a.do_dit = s.do_dit;
+    a.unpermute = s.unpermute;
+    a.mid_on = s.mid_on;
+    a.pre_v = s.pre_v;
+    a.post_v = s.post_v;
+    a.nrep = s.nrep;
+    a.vtab = plan->d_vtab;
+    a.vrep = plan->vrep;
+    a.v_mid_full = s.v_mid_full;
+    a.ephase = nullptr;
+    a.step_avg = plan->d_avg;
+    a.field_kind = plan->field_kind;
+    a.ndim = plan->ndim;
+    a.line_axis = s.axis;
+    a.n0 = s.n;
+    a.half_dt = 0.5 * plan->dt;
+    a.dt = plan->dt;
+    for (int i = 0; i < 3; ++i) {
+        a.nsz[i] = i < plan->ndim ? plan->ax[i].n : 1;
+        a.dxs[i] = i < plan->ndim ? plan->ax[i].dx : 1.0;
+    }
+    a.mass = plan->mass;
+    a.clight = plan->clight;
+    a.charge = plan->charge;
+    a.scale = 1.0 / (double)plan->npts;
+    if (s.pw == PW_KS) {
+        a.kph0 = A.d_kph;
+        a.kph1 = g.oaxA >= 0 ? plan->ax[g.oaxA].d_kph : nullptr;
+        a.kph2 = g.oaxB >= 0 ? plan->ax[g.oaxB].d_kph : nullptr;
+    } else if (s.pw == PW_KD2 || s.pw == PW_KD4) {
+        a.kv0 = A.d_kv;
+        a.kv1 = g.oaxA >= 0 ? plan->ax[g.oaxA].d_kv : nullptr;
+        a.kv2 = g.oaxB >= 0 ? plan->ax[g.oaxB].d_kv : nullptr;
+    } else if (s.pw == PW_V && s.mid_on && plan->field_kind == SSO_FIELD_E && plan->e_along_last) {
+        // phase of the field component along the line, rebuilt for this step (prep kernel)
+        const int blocks = (A.n + 127) / 128;
+        if (plan->precision == SSO_C128)
+            build_ephase_kernel<double><<<blocks, 128, 0, st>>>(A.d_ephase, A.n, A.d_slot_nat, A.dx, 0.5 * plan->dt, plan->d_avg, s.n, s.n + 1, s.v_mid_full, plan->ndim, s.axis);
+        else
+            build_ephase_kernel<float><<<blocks, 128, 0, st>>>(A.d_ephase, A.n, A.d_slot_nat, A.dx, 0.5 * plan->dt, plan->d_avg, s.n, s.n + 1, s.v_mid_full, plan->ndim, s.axis);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(plan, e, "ephase kernel");
+        a.ephase = A.d_ephase;
+    }
+    LaunchFn fn = find_launch(plan->precision, A.n, g.strided ? 1 : 0, s.pw, s.sign);
+    if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no kernel built for this pass");
+    const long long tiles = g.lines / TL;
+    const long long grid = cc == 1 ? tiles * plan->ncomp : tiles;
+    const unsigned threads = (unsigned)(cc * TL * U);
+    const size_t smem = (size_t)cc * TL * pitch * esz + (size_t)TL * esz + (size_t)TL * 2 * sizeof(double);
+    cudaError_t e = fn(a, (unsigned)grid, threads, smem, st);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "pass kernel launch");
+    return SSO_OK;
+}
+
+// (re)build the Schroedinger kinetic phase tables; with SSO_FIELD_A they depend on the step
+int build_kphase(sso_plan *plan, long long n, cudaStream_t st) {
+    const bool shifted = plan->field_kind == SSO_FIELD_A;
+    if (plan->kph_valid && !shifted) return SSO_OK;
+    for (int a = 0; a < plan->ndim; ++a) {
+        Axis &A = plan->ax[a];
+        const double scale = a == 0 ? 1.0 / (double)plan->npts : 1.0;
+        const int blocks = (A.n + 127) / 128;
+        if (plan->precision == SSO_C128)
+            build_kphase_kernel<double><<<blocks, 128, 0, st>>>(A.d_kv, A.d_kph, A.n, plan->dt, plan->mass, shifted ? plan->d_avg : nullptr, n, plan->ndim, a, plan->charge, scale);
+        else
+            build_kphase_kernel<float><<<blocks, 128, 0, st>>>(A.d_kv, A.d_kph, A.n, plan->dt, plan->mass, shifted ? plan->d_avg : nullptr, n, plan->ndim, a, plan->charge, scale);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(plan, e, "kinetic phase kernel");
+    }
+    plan->kph_valid = !shifted;
+    return SSO_OK;
+}
+
+int kinetic_pw(const sso_plan *p) { return p->ncomp == 1 ? PW_KS : (p->ncomp == 2 ? PW_KD2 : PW_KD4); }
+
+long long launches_for(const sso_plan *p, long long nsteps) {
+    if (nsteps <= 0) return 0;
+    long long cnt = 0;
+    const bool kshift = p->ncomp == 1 && p->field_kind == SSO_FIELD_A;
+    const bool kbuild = p->ncomp == 1 && (kshift || !p->kph_valid);
+    if (p->ndim == 1) {
+        if (kshift) return nsteps * (1 + p->ndim);
+        return 1 + (kbuild ? p->ndim : 0);
+    }
+    const bool eph = p->field_kind == SSO_FIELD_E && p->e_along_last;
+    cnt += 1;                                    // opening
+    cnt += nsteps * (p->ndim == 3 ? 3 : 1);      // kinetic sandwich (+ middle-axis DIF and DIT)
+    cnt += nsteps * (eph ? 2 : 1);               // potential sandwiches and the closing pass
+    if (kshift) cnt += nsteps * p->ndim;
+    else if (kbuild) cnt += p->ndim;
+    return cnt;
+}
+
+}  // namespace
+
+extern "C" {
+
+int sso_launch_count(const sso_plan *plan, int64_t nsteps, int64_t *count) {
+    if (!plan || !count) return SSO_ERR_INVALID;
+    *count = launches_for(plan, nsteps);
+    return SSO_OK;
+}
+
+int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (!psi) return fail(plan, SSO_ERR_INVALID, "psi is NULL");
+    if (((uintptr_t)psi & 15u) != 0) return fail(plan, SSO_ERR_INVALID, "psi must be 16-byte aligned");
+    if (nsteps < 0) return fail(plan, SSO_ERR_INVALID, "nsteps must be >= 0");
+    if (nsteps == 0) return SSO_OK;
+    if (plan->field_kind != SSO_FIELD_NONE && plan->tindex + nsteps > plan->nvals)
+        return fail(plan, SSO_ERR_STATE, "field table shorter than the steps requested");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int nd = plan->ndim;
+    const int kpw = kinetic_pw(plan);
+    const long long n0 = plan->tindex;
+    int rc;
+    if (nd == 1) {
+        // one persistent CTA: V/2, then nsteps x [F K F^-1, V (merged) or V/2 (last)]
+        const bool kshift = plan->ncomp == 1 && plan->field_kind == SSO_FIELD_A;
+        const long long chunk = kshift ? 1 : nsteps;  // step-dependent kinetic tables force one launch per step
+        for (long long s = 0; s < nsteps; s += chunk) {
+            if (plan->ncomp == 1 && (rc = build_kphase(plan, n0 + s, st)) != SSO_OK) return rc;
+            PassSpec ps{0, kpw, -1, 1, 1, 0, 1, 1, 1, 0, (int)chunk, n0 + s};
+            if (chunk > 0x7fffffffLL) return fail(plan, SSO_ERR_INVALID, "nsteps too large");
+            if ((rc = launch(plan, psi, ps, st)) != SSO_OK) return rc;
+        }
+    } else {
+        const int last = nd - 1;
+        // opening: V/2 in natural order, forward transform along the last axis, natural frequency order out
+        PassSpec open{last, PW_NONE, -1, 1, 0, 1, 0, 2, 0, 0, 1, n0};
+        if ((rc = launch(plan, psi, open, st)) != SSO_OK) return rc;
+        for (long long s = 0; s < nsteps; ++s) {
+            const long long n = n0 + s;
+            if (plan->ncomp == 1 && (rc = build_kphase(plan, n, st)) != SSO_OK) return rc;
+            if (nd == 3) {
+                PassSpec mid{1, PW_NONE, -1, 1, 0, 0, 0, 0, 0, 0, 1, n};  // F_1, stored in network order
+                if ((rc = launch(plan, psi, mid, st)) != SSO_OK) return rc;
+            }
+            PassSpec kin{0, kpw, -1, 1, 1, 0, 1, 0, 0, 0, 1, n};  // F_0 K F_0^-1
+            if ((rc = launch(plan, psi, kin, st)) != SSO_OK) return rc;
+            if (nd == 3) {
+                PassSpec mid{1, PW_NONE, -1, 0, 1, 0, 0, 0, 0, 0, 1, n};  // F_1^-1 from network order
+                if ((rc = launch(plan, psi, mid, st)) != SSO_OK) return rc;
+            }
+            if (s + 1 < nsteps) {
+                PassSpec pot{last, PW_V, +1, 1, 1, 0, 1, 0, 0, 1, 1, n};  // F_last^-1 V(n, n+1) F_last
+                if ((rc = launch(plan, psi, pot, st)) != SSO_OK) return rc;
+            } else {
+                PassSpec close{last, PW_V, +1, 1, 0, 1, 1, 0, 0, 0, 1, n};  // F_last^-1, V/2, natural order out
+                if ((rc = launch(plan, psi, close, st)) != SSO_OK) return rc;
+            }
+        }
+    }
+    plan->tindex += nsteps;
+    return SSO_OK;
+}
+
+int sso_step_host(sso_plan *plan, void *psi_host, int64_t nsteps) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (!psi_host) return fail(plan, SSO_ERR_INVALID, "psi_host is NULL");
+    if (nsteps < 0) return fail(plan, SSO_ERR_INVALID, "nsteps must be >= 0");
+    const size_t bytes = (size_t)plan->npts * plan->ncomp * plan->esize();
+    if (!plan->d_hostbuf) {
+        cudaError_t e = cudaMalloc(&plan->d_hostbuf, bytes);
+        if (e != cudaSuccess) return fail(plan, SSO_ERR_ALLOC, std::string("device buffer: ") + cudaGetErrorString(e));
+    }
+    CK(cudaMemcpy(plan->d_hostbuf, psi_host, bytes, cudaMemcpyHostToDevice));
+    int rc = sso_step(plan, plan->d_hostbuf, nsteps, nullptr);
+    if (rc != SSO_OK) return rc;
+    CK(cudaMemcpy(psi_host, plan->d_hostbuf, bytes, cudaMemcpyDeviceToHost));
+    return SSO_OK;
+}
+
+int sso_norm(sso_plan *plan, const void *psi, double *out_host, void *stream) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (!psi || !out_host) return fail(plan, SSO_ERR_INVALID, "psi or out_host is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long count = plan->npts * plan->ncomp;
+    double vol = 1.0;
+    for (int a = 0; a < plan->ndim; ++a) vol *= plan->ax[a].dx;
+    if (plan->precision == SSO_C128)
+        norm_partial_kernel<double><<<NORM_BLOCKS, 256, 0, st>>>(psi, count, plan->d_partial);
+    else
+        norm_partial_kernel<float><<<NORM_BLOCKS, 256, 0, st>>>(psi, count, plan->d_partial);
+    norm_final_kernel<<<1, 32, 0, st>>>(plan->d_partial, NORM_BLOCKS, vol, plan->d_norm);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(out_host, plan->d_norm, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return SSO_OK;
+}
+
+}  // extern "C"

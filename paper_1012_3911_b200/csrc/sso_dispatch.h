@@ -1,0 +1,67 @@
+// sso_dispatch.h -- pass descriptor shared by the kernels (sso_pass.cuh), their per-size
+// instantiations (sso_inst.cu) and the host-side plan (sso_api.cu).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sso {
+
+enum : int { PW_NONE = 0, PW_V = 1, PW_KS = 2, PW_KD2 = 3, PW_KD4 = 4 };
+
+// V-phase representation
+enum : int { VREP_TABLE = 0, VREP_ANGLE = 1 };
+
+struct PassArgs {
+    void *psi;               // device, [ncomp][...] complex
+    const void *tw;          // complex[N]: exp(-2 pi i t / N)
+    const int *revB;         // int[N/16]: digit reversal of the last-stage thread index
+    const int *revBinv;      // int[N/16]: its inverse
+    long long comp_stride;   // complex elements between components
+    long long inner;         // element stride along the line (1 = contiguous axis)
+    int ncomp;               // components in psi
+    int TL;                  // lines per component per CTA
+    int pitch;               // shared-memory line pitch in complex elements
+    int rest1;               // size of the faster non-line axis: line index = ia * rest1 + ib, >= 1
+    int oaxA, oaxB;          // lattice axes that ia and ib run along (-1: absent)
+    // structure of the pass
+    int do_dif, do_dit, unpermute;
+    int mid_on;              // apply the pointwise factor between DIF and DIT
+    int pre_v, post_v;       // 0 none; 1 natural-order table (1D); 2 gather from the permuted table (opening pass)
+    int nrep;                // repetitions inside the kernel (1D persistent stepping), >= 1
+    // potential phase
+    const void *vtab;        // complex h = exp(-i V tau/2) (VREP_TABLE) or real angle -V tau/2 (VREP_ANGLE)
+    int vrep;
+    int v_mid_full;          // mid factor is the full (merged) phase h^2
+    const void *ephase;      // complex[N] extra phase along the line (permuted layout) or NULL
+    // field table
+    const double *step_avg;  // device [nvals][ndim] or NULL
+    int field_kind;          // SSO_FIELD_*
+    int ndim;
+    int line_axis;           // which lattice axis the lines run along
+    long long n0;            // step index of the first repetition
+    double half_dt;          // tau/2
+    double dt;               // tau
+    int nsz[3];              // lattice sizes
+    double dxs[3];           // lattice spacings
+    // kinetic factor
+    const void *kph0;        // Schroedinger: complex[N] line-axis phase table incl. 1/Ntot, permuted layout
+    const void *kph1;        // complex[rest0] storage-order table of the slower non-line axis or NULL
+    const void *kph2;        // complex[rest1] table of the faster non-line axis or NULL
+    const double *kv0;       // Dirac: k values along the line (permuted layout)
+    const double *kv1;       // k values, slower non-line axis (storage order) or NULL
+    const double *kv2;       // k values, faster non-line axis or NULL
+    double mass, clight, charge;
+    double scale;            // 1/Ntot (Dirac; Schroedinger folds it into kph0)
+};
+
+using LaunchFn = cudaError_t (*)(const PassArgs &, unsigned grid, unsigned threads, size_t smem, cudaStream_t st);
+
+// one lookup function per compiled (precision, line length); returns NULL for a variant that is not built
+#define SSO_FOR_EACH_N(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096)
+#define SSO_DECL_LOOKUP(N)                                         \
+    LaunchFn sso_lookup_f32_##N(int strided, int pw, int sign);    \
+    LaunchFn sso_lookup_f64_##N(int strided, int pw, int sign);
+SSO_FOR_EACH_N(SSO_DECL_LOOKUP)
+#undef SSO_DECL_LOOKUP
+
+}  // namespace sso

@@ -1,0 +1,53 @@
+// sso_inst.cu -- explicit instantiations of the pass kernel for one (precision, line length).
+// Compiled once per pair with -DSSO_T=<float|double> -DSSO_TNAME=<f32|f64> -DSSO_N=<n>
+// (see paper_1012_3911_b200/build.py); each object exports one lookup function that the
+// dispatcher in sso_api.cu calls.
+#include "sso_pass.cuh"
+#include "sso_dispatch.h"
+
+#ifndef SSO_T
+#error "compile with -DSSO_T=float|double -DSSO_TNAME=f32|f64 -DSSO_N=<line length>"
+#endif
+
+namespace sso {
+
+template <typename T, int N, bool STRIDED, int PW, int SIGN>
+cudaError_t launch_pass(const PassArgs &a, unsigned grid, unsigned threads, size_t smem, cudaStream_t st) {
+    auto kern = pass_kernel<T, N, STRIDED, PW, SIGN>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    kern<<<grid, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+#define SSO_CAT3_(a, b, c) a##b##_##c
+#define SSO_CAT3(a, b, c) SSO_CAT3_(a, b, c)
+
+#ifdef SSO_STUB
+// development builds may leave a size out (SSO_SIZES in build.py): the dispatcher then reports "unsupported"
+LaunchFn SSO_CAT3(sso_lookup_, SSO_TNAME, SSO_N)(int, int, int) { return nullptr; }
+#else
+LaunchFn SSO_CAT3(sso_lookup_, SSO_TNAME, SSO_N)(int strided, int pw, int sign) {
+    using T = SSO_T;
+    constexpr int N = SSO_N;
+    if (!strided) {
+        if (pw == PW_V && sign > 0) return &launch_pass<T, N, false, PW_V, +1>;      // potential sandwich, closing pass
+        if (pw == PW_NONE && sign < 0) return &launch_pass<T, N, false, PW_NONE, -1>;  // opening pass
+        if (pw == PW_KS && sign < 0) return &launch_pass<T, N, false, PW_KS, -1>;     // 1D step
+        if (pw == PW_KD2 && sign < 0) return &launch_pass<T, N, false, PW_KD2, -1>;
+        if (pw == PW_KD4 && sign < 0) return &launch_pass<T, N, false, PW_KD4, -1>;
+    } else {
+        if (pw == PW_NONE && sign < 0) return &launch_pass<T, N, true, PW_NONE, -1>;   // middle-axis DIF / DIT
+        if (pw == PW_KS && sign < 0) return &launch_pass<T, N, true, PW_KS, -1>;      // kinetic sandwich
+        if (pw == PW_KD2 && sign < 0) return &launch_pass<T, N, true, PW_KD2, -1>;
+        if (pw == PW_KD4 && sign < 0) return &launch_pass<T, N, true, PW_KD4, -1>;
+    }
+    return nullptr;
+}
+#endif
+
+}  // namespace sso

@@ -1,0 +1,502 @@
+// sso_pass.cuh -- the line-pass kernel of the split-operator step (sm_100a).
+//
+// One CTA holds a tile of whole lattice lines on chip and applies, without
+// leaving the SM,
+//
+//     [pre-phase]  ->  DIF FFT (sign s)  ->  [pointwise factor]  ->  DIT FFT (sign -s)  ->  [post-phase]
+//
+// to every line of the tile.  The pointwise factor is the potential phase of
+// PAPER.md:98 (eq. 11), the Schroedinger kinetic phase of PAPER.md:107 (eq. 13)
+// or the Dirac kinetic unitary of PAPER.md:203-232 (eq. 27-33) in the closed form
+// U = cos(E tau) - i sin(E tau)/E (c alpha.pi + m c^2 beta), which follows from
+// H^2 = E^2 by the argument of PAPER.md:168-184 (eq. 23/24).
+// ("Kernels") for the data layout, the radix schedule and the byte counts.
+//
+// FFT structure.  A line of N = R_1 R_2 ... R_m points (R_m = 16, the other R_i
+// in {2,4,8,16}) is transformed by an in-place decimation-in-frequency network
+// (natural order in, mixed-radix digit-reversed order out) and transformed back
+// by the transposed decimation-in-time network (digit-reversed in, natural out),
+// so no reordering pass is ever needed: the pointwise tables are stored in the
+// digit-reversed order instead.  Every thread holds 16 complex points in
+// registers in every stage; a radix-R stage is 16/R register butterflies; between
+// stages the points are exchanged through padded shared memory.  The first stage
+// reads global memory directly into registers and the last stage writes it back.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "sso_dispatch.h"
+
+namespace sso {
+
+template <typename T> struct CxOf;
+template <> struct CxOf<float> { using type = float2; };
+template <> struct CxOf<double> { using type = double2; };
+
+template <typename C> __device__ __forceinline__ C mk(decltype(C::x) a, decltype(C::x) b) {
+    C r;
+    r.x = a;
+    r.y = b;
+    return r;
+}
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { return mk<C>(a.x + b.x, a.y + b.y); }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { return mk<C>(a.x - b.x, a.y - b.y); }
+template <typename C> __device__ __forceinline__ C cmul(C a, C b) {
+    return mk<C>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+template <typename C> __device__ __forceinline__ C cmulc(C a, C b) {  // a * conj(b)
+    return mk<C>(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+
+// ------------------------------------------------------------------------------------------
+// radix schedule: N = 2^LOG, last stage radix 16, the LOG-4 remaining bits in stages of <= 4 bits,
+// the first stage taking the remainder.
+// ------------------------------------------------------------------------------------------
+__host__ __device__ constexpr int ilog2c(int n) { return n <= 1 ? 0 : 1 + ilog2c(n >> 1); }
+
+template <int N> struct Sched {
+    static constexpr int LOG = ilog2c(N);
+    static_assert((1 << LOG) == N && LOG >= 4, "N must be a power of two >= 16");
+    static constexpr int REM = LOG - 4;
+    static constexpr int M = 1 + (REM + 3) / 4;  // number of stages
+    __host__ __device__ static constexpr int lr(int i) { return i == M - 1 ? 4 : (i == 0 ? REM - 4 * (M - 2) : 4); }
+    __host__ __device__ static constexpr int nprev(int i) {  // length of the sub-transform entering stage i
+        int n = N;
+        for (int j = 0; j < i; ++j) n >>= lr(j);
+        return n;
+    }
+};
+
+// cos(2 pi j/16), sin(2 pi j/16), j = 0..7
+__host__ __device__ constexpr double cos16(int j) {
+    return j == 0 ? 1.0
+         : j == 1 ? 0.92387953251128675613
+         : j == 2 ? 0.70710678118654752440
+         : j == 3 ? 0.38268343236508977173
+         : j == 4 ? 0.0
+         : j == 5 ? -0.38268343236508977173
+         : j == 6 ? -0.70710678118654752440
+                  : -0.92387953251128675613;
+}
+__host__ __device__ constexpr double sin16(int j) {
+    return j == 0 ? 0.0
+         : j == 1 ? 0.38268343236508977173
+         : j == 2 ? 0.70710678118654752440
+         : j == 3 ? 0.92387953251128675613
+         : j == 4 ? 1.0
+         : j == 5 ? 0.92387953251128675613
+         : j == 6 ? 0.70710678118654752440
+                  : 0.38268343236508977173;
+}
+
+// v * exp(SIGN 2 pi i j / R), j < R/2, all compile-time after unrolling
+template <int R, int SIGN, typename C> __device__ __forceinline__ C mul_root(C v, int j) {
+    using T = decltype(C::x);
+    const int j16 = j * (16 / R);
+    if (j16 == 0) return v;
+    if (j16 == 4) return SIGN > 0 ? mk<C>(-v.y, v.x) : mk<C>(v.y, -v.x);
+    const T c = (T)cos16(j16);
+    const T s = (T)(SIGN > 0 ? sin16(j16) : -sin16(j16));
+    return mk<C>(v.x * c - v.y * s, v.x * s + v.y * c);
+}
+
+__host__ __device__ constexpr int brevc(int k, int bits) {
+    int r = 0;
+    for (int b = 0; b < bits; ++b) r |= ((k >> b) & 1) << (bits - 1 - b);
+    return r;
+}
+
+// radix-2 decimation-in-frequency recursion on x[j*S], j < R; output bit-reversed
+template <int R, int S, int SIGN, typename C> __device__ __forceinline__ void dif_rec(C *x) {
+    if constexpr (R >= 2) {
+        constexpr int H = R / 2;
+#pragma unroll
+        for (int j = 0; j < H; ++j) {
+            C a = x[j * S], b = x[(j + H) * S];
+            x[j * S] = cadd(a, b);
+            x[(j + H) * S] = mul_root<R, SIGN>(csub(a, b), j);
+        }
+        dif_rec<H, S, SIGN>(x);
+        dif_rec<H, S, SIGN>(x + H * S);
+    }
+}
+
+// y[k*S] = sum_j x[j*S] exp(SIGN 2 pi i j k / R), natural order in and out, in registers
+template <int R, int S, int SIGN, typename C> __device__ __forceinline__ void dft_reg(C *x) {
+    dif_rec<R, S, SIGN>(x);
+    if constexpr (R > 2) {
+        constexpr int B = ilog2c(R);
+        C t[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) t[k] = x[brevc(k, B) * S];
+#pragma unroll
+        for (int k = 0; k < R; ++k) x[k * S] = t[k];
+    }
+}
+
+// position (within the line) of register q of thread u in the layout of stage I:
+//   u = B' * Mi + l',  pos = B' * 16 Mi + q Mi + l',  Mi = nprev(I)/16
+template <int N, int I> __device__ __forceinline__ int stage_pos(int u, int q) {
+    constexpr int Mi = Sched<N>::nprev(I) / 16;
+    return (u / Mi) * (16 * Mi) + q * Mi + (u % Mi);
+}
+__device__ __forceinline__ int padp(int p) { return p + (p >> 4); }
+
+// one DIF stage: butterflies over the top digit of the current sub-transform, then twiddles
+template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void dif_stage(typename CxOf<T>::type (&x)[16], int u, const typename CxOf<T>::type *__restrict__ tw) {
+    using C = typename CxOf<T>::type;
+    constexpr int R = 1 << Sched<N>::lr(I);
+    constexpr int NP = Sched<N>::nprev(I);
+    constexpr int Mi = NP / 16;
+    constexpr int S = 16 / R;
+#pragma unroll
+    for (int s = 0; s < S; ++s) dft_reg<R, S, SIGN>(&x[s]);
+    if constexpr (NP > R) {
+        constexpr int TS = N / NP;
+        const int lp = u % Mi;
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            const int l = s * Mi + lp;
+#pragma unroll
+            for (int k = 1; k < R; ++k) {
+                const C w = __ldg(&tw[l * k * TS]);
+                x[k * S + s] = SIGN < 0 ? cmul(x[k * S + s], w) : cmulc(x[k * S + s], w);
+            }
+        }
+    }
+}
+
+// the transposed (DIT) stage: twiddles, then butterflies
+template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void dit_stage(typename CxOf<T>::type (&x)[16], int u, const typename CxOf<T>::type *__restrict__ tw) {
+    using C = typename CxOf<T>::type;
+    constexpr int R = 1 << Sched<N>::lr(I);
+    constexpr int NP = Sched<N>::nprev(I);
+    constexpr int Mi = NP / 16;
+    constexpr int S = 16 / R;
+    if constexpr (NP > R) {
+        constexpr int TS = N / NP;
+        const int lp = u % Mi;
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            const int l = s * Mi + lp;
+#pragma unroll
+            for (int k = 1; k < R; ++k) {
+                const C w = __ldg(&tw[l * k * TS]);
+                x[k * S + s] = SIGN < 0 ? cmul(x[k * S + s], w) : cmulc(x[k * S + s], w);
+            }
+        }
+    }
+#pragma unroll
+    for (int s = 0; s < S; ++s) dft_reg<R, S, SIGN>(&x[s]);
+}
+
+// registers (layout of stage IA) -> shared memory -> registers (layout of stage IB)
+template <typename T, int N, int IA, int IB> __device__ __forceinline__ void exchange(typename CxOf<T>::type (&x)[16], int u, typename CxOf<T>::type *sl) {
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 16; ++q) sl[padp(stage_pos<N, IA>(u, q))] = x[q];
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 16; ++q) x[q] = sl[padp(stage_pos<N, IB>(u, q))];
+}
+
+template <typename T, int N, int I, int SIGN> struct DifChain {
+    using C = typename CxOf<T>::type;
+    static __device__ __forceinline__ void run(C (&x)[16], int u, const C *tw, C *sl) {
+        dif_stage<T, N, I, SIGN>(x, u, tw);
+        if constexpr (I + 1 < Sched<N>::M) {
+            exchange<T, N, I, I + 1>(x, u, sl);
+            DifChain<T, N, I + 1, SIGN>::run(x, u, tw, sl);
+        }
+    }
+};
+template <typename T, int N, int I, int SIGN> struct DitChain {  // runs stages I, I-1, ..., 0
+    using C = typename CxOf<T>::type;
+    static __device__ __forceinline__ void run(C (&x)[16], int u, const C *tw, C *sl) {
+        dit_stage<T, N, I, SIGN>(x, u, tw);
+        if constexpr (I > 0) {
+            exchange<T, N, I, I - 1>(x, u, sl);
+            DitChain<T, N, I - 1, SIGN>::run(x, u, tw, sl);
+        }
+    }
+};
+
+// exp(i a) for a phase table entry or an angle, in the working precision
+template <typename T> __device__ __forceinline__ typename CxOf<T>::type expi(double a) {
+    double s, c;
+    sincos(a, &s, &c);
+    return mk<typename CxOf<T>::type>((T)c, (T)s);
+}
+
+// step average row n, component a (0 when there is no table)
+__device__ __forceinline__ double favg(const PassArgs &a, long long n, int ax) {
+    return a.step_avg ? a.step_avg[n * a.ndim + ax] : 0.0;
+}
+
+// ------------------------------------------------------------------------------------------
+// the kernel
+//   STRIDED = false: lines are contiguous in memory; a tile is TL consecutive lines.
+//   STRIDED = true : consecutive line elements are `inner` apart; a tile is TL adjacent lines
+//                    (TL * sizeof(complex) contiguous bytes per line element).
+//   PW: pointwise factor kind.  The Dirac kinds hold all components of the tile's lines in one CTA.
+//   SIGN: sign of the DIF transform (-1: forward first, the kinetic sandwich; +1: inverse first,
+//         the potential sandwich).
+// ------------------------------------------------------------------------------------------
+template <typename T, int N, bool STRIDED, int PW, int SIGN>
+__global__ void __launch_bounds__(512) pass_kernel(const PassArgs a) {
+    using C = typename CxOf<T>::type;
+    constexpr int U = N / 16;
+    constexpr int CC = PW == PW_KD2 ? 2 : (PW == PW_KD4 ? 4 : 1);
+    constexpr int LAST = Sched<N>::M - 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *sm = reinterpret_cast<C *>(smem_raw);
+
+    const int TL = a.TL;
+    const int tid = threadIdx.x;
+    int t, c, u;
+    if (STRIDED) {
+        t = tid % TL;
+        const int cu = tid / TL;
+        u = cu % U;
+        c = cu / U;
+    } else {
+        u = tid % U;
+        const int ct = tid / U;
+        t = ct % TL;
+        c = ct / TL;
+    }
+    long long tile;
+    int comp;
+    if (CC == 1) {
+        comp = (int)(blockIdx.x % (unsigned)a.ncomp);
+        tile = blockIdx.x / (unsigned)a.ncomp;
+    } else {
+        comp = c;
+        tile = blockIdx.x;
+    }
+    const long long line = tile * TL + t;  // line index within a component
+    long long base, estep;
+    if (STRIDED) {
+        const long long o = line / a.inner, i = line % a.inner;
+        base = o * (long long)N * a.inner + i;
+        estep = a.inner;
+    } else {
+        base = line * (long long)N;
+        estep = 1;
+    }
+    C *__restrict__ gp = reinterpret_cast<C *>(a.psi) + (long long)comp * a.comp_stride + base;
+    C *sl = sm + (c * TL + t) * a.pitch;
+    C *lsc = sm + CC * TL * a.pitch;  // per-line scalars [TL] (complex) ...
+    double *lkv = reinterpret_cast<double *>(lsc + TL);  // ... and per-line k values [TL][2] (Dirac)
+    const C *__restrict__ tw = reinterpret_cast<const C *>(a.tw);
+
+    // line coordinates on the non-line axes: line = ia * rest1 + ib
+    const int ib = (int)(line % a.rest1);
+    const int ia = (int)(line / a.rest1);
+
+    // per-line kinetic scalars
+    if (PW == PW_KS && (a.kph1 || a.kph2)) {
+        if (u == 0 && c == 0) {
+            C s = mk<C>((T)1, (T)0);
+            if (a.kph1) s = reinterpret_cast<const C *>(a.kph1)[ia];
+            if (a.kph2) s = a.kph1 ? cmul(s, reinterpret_cast<const C *>(a.kph2)[ib]) : reinterpret_cast<const C *>(a.kph2)[ib];
+            lsc[t] = s;
+        }
+    }
+
+    C x[16];
+    if (a.do_dif) {
+#pragma unroll
+        for (int q = 0; q < 16; ++q) x[q] = gp[(long long)(u + q * U) * estep];
+    } else {
+#pragma unroll
+        for (int q = 0; q < 16; ++q) x[q] = gp[(long long)(u * 16 + q) * estep];
+    }
+
+    // angle of the homogeneous-field phase contributed by the non-line axes of this line:
+    // (tau/2) sum_ax (Ebar_na + [full] Ebar_nb)[ax] * r_ax      (eq. 11, reading G12)
+    auto other_axes_angle = [&](long long n_a, long long n_b, bool full) -> double {
+        double ang = 0.0;
+        if (a.oaxA >= 0) {
+            double e = favg(a, n_a, a.oaxA);
+            if (full) e += favg(a, n_b, a.oaxA);
+            ang += e * a.half_dt * ((double)ia - (double)(a.nsz[a.oaxA] / 2)) * a.dxs[a.oaxA];
+        }
+        if (a.oaxB >= 0) {
+            double e = favg(a, n_a, a.oaxB);
+            if (full) e += favg(a, n_b, a.oaxB);
+            ang += e * a.half_dt * ((double)ib - (double)(a.nsz[a.oaxB] / 2)) * a.dxs[a.oaxB];
+        }
+        return ang;
+    };
+
+    // potential phase in natural order at the stage-0 layout (thread u holds positions u + q U);
+    // mode 1: the table is in natural order (1D); mode 2: gather from the permuted table
+    auto natural_v = [&](int mode, long long n_a, long long n_b, bool full) {
+        if constexpr (!STRIDED) {
+            const int slot_u = mode == 2 ? a.revBinv[u] : u;
+            double gl = 0.0, gother = 0.0;
+            if (a.field_kind == 1) {
+                double e = favg(a, n_a, a.line_axis);
+                if (full) e += favg(a, n_b, a.line_axis);
+                gl = e * a.half_dt;
+                gother = other_axes_angle(n_a, n_b, full);
+            }
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                C h;
+                const long long vi = line * (long long)N + q * U + slot_u;
+                if (a.vrep == VREP_TABLE) {
+                    h = reinterpret_cast<const C *>(a.vtab)[vi];
+                    if (full) h = cmul(h, h);
+                } else {
+                    const double ang = reinterpret_cast<const double *>(a.vtab)[vi];
+                    h = expi<T>(full ? 2.0 * ang : ang);
+                }
+                if (a.field_kind == 1) {
+                    const double r = ((double)(u + q * U) - (double)(N / 2)) * a.dxs[a.line_axis];
+                    h = cmul(h, expi<T>(-(gl * r + gother)));
+                }
+                x[q] = cmul(x[q], h);
+            }
+        }
+    };
+
+    for (int rep = 0; rep < a.nrep; ++rep) {
+        const long long n = a.n0 + rep;
+        if (a.pre_v && rep == 0) natural_v(a.pre_v, n, n, false);
+
+        if (a.do_dif) DifChain<T, N, 0, SIGN>::run(x, u, tw, sl);
+
+        if (a.mid_on) {
+            if constexpr (PW == PW_V) {
+                // merged or half potential phase in the permuted order: register q of thread u is
+                // table slot q U + u (coalesced across u)
+                if (a.field_kind == 1 && u == 0) lsc[t] = expi<T>(-other_axes_angle(n, n + 1, a.v_mid_full != 0));
+                if (a.field_kind == 1) __syncthreads();
+                const long long vb = line * (long long)N + u;
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    C h;
+                    if (a.vrep == VREP_TABLE) {
+                        h = reinterpret_cast<const C *>(a.vtab)[vb + q * U];
+                        if (a.v_mid_full) h = cmul(h, h);
+                    } else {
+                        const double ang = reinterpret_cast<const double *>(a.vtab)[vb + q * U];
+                        h = expi<T>(a.v_mid_full ? 2.0 * ang : ang);
+                    }
+                    if (a.field_kind == 1) h = cmul(h, lsc[t]);
+                    if (a.ephase) h = cmul(h, reinterpret_cast<const C *>(a.ephase)[q * U + u]);
+                    x[q] = cmul(x[q], h);
+                }
+            } else if constexpr (PW == PW_KS) {
+                const bool has_lsc = a.kph1 || a.kph2;
+                if (has_lsc && Sched<N>::M == 1) __syncthreads();
+                const C *__restrict__ k0 = reinterpret_cast<const C *>(a.kph0);
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    C f = k0[q * U + u];
+                    if (has_lsc) f = cmul(f, lsc[t]);
+                    x[q] = cmul(x[q], f);
+                }
+            } else if constexpr (PW == PW_KD2 || PW == PW_KD4) {
+                constexpr int PP = 16 / CC;
+                // shift of the kinetic momentum: pi = k - q Abar_n (reading G16)
+                double sh[3] = {0.0, 0.0, 0.0};
+                if (a.field_kind == 2)
+                    for (int ax = 0; ax < a.ndim; ++ax) sh[ax] = a.charge * favg(a, n, ax);
+                // non-line momenta of this line: the line axis is axis 0 here
+                double p1 = 0.0, p2 = 0.0;
+                if (a.ndim == 2) p1 = a.kv2[ib] - sh[1];
+                if (a.ndim == 3) {
+                    p1 = a.kv1[ia] - sh[1];
+                    p2 = a.kv2[ib] - sh[2];
+                }
+                __syncthreads();
+#pragma unroll
+                for (int q = 0; q < 16; ++q) sl[padp(u * 16 + q)] = x[q];
+                __syncthreads();
+                C y[CC][PP];
+#pragma unroll
+                for (int c2 = 0; c2 < CC; ++c2)
+#pragma unroll
+                    for (int i = 0; i < PP; ++i) y[c2][i] = sm[(c2 * TL + t) * a.pitch + padp(u * 16 + c * PP + i)];
+                const double mc2 = a.mass * a.clight * a.clight;
+#pragma unroll
+                for (int i = 0; i < PP; ++i) {
+                    const int q2 = c * PP + i;
+                    const double p0 = a.kv0[q2 * U + u] - sh[0];
+                    const double pp = p0 * p0 + p1 * p1 + p2 * p2;
+                    const double E = sqrt(a.clight * a.clight * pp + mc2 * mc2);
+                    double sn, cs;
+                    sincos(E * a.dt, &sn, &cs);
+                    double sE = E > 0.0 ? sn / E : a.dt;
+                    cs *= a.scale;
+                    sE *= a.scale;
+                    const T fc = (T)cs;
+                    const T fm = (T)(sE * mc2);
+                    const T f0 = (T)(sE * a.clight * p0), f1 = (T)(sE * a.clight * p1), f2 = (T)(sE * a.clight * p2);
+                    // out = cs psi - i sE H psi ;  (-i)(a + i b) = b - i a
+                    if constexpr (CC == 2) {
+                        const C a0 = y[0][i], a1 = y[1][i];
+                        // H psi_0 = mc2 a0 + c (p0 - i p1) a1 ; H psi_1 = c (p0 + i p1) a0 - mc2 a1
+                        const C h0 = mk<C>(fm * a0.x + f0 * a1.x + f1 * a1.y, fm * a0.y + f0 * a1.y - f1 * a1.x);
+                        const C h1 = mk<C>(f0 * a0.x - f1 * a0.y - fm * a1.x, f0 * a0.y + f1 * a0.x - fm * a1.y);
+                        y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
+                        y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
+                    } else {
+                        const C a0 = y[0][i], a1 = y[1][i], a2 = y[2][i], a3 = y[3][i];
+                        // sigma.p (v0, v1) = (p2 v0 + (p0 - i p1) v1, (p0 + i p1) v0 - p2 v1)
+                        // H psi = (mc2 u + c sigma.p l, c sigma.p u - mc2 l)
+                        const C h0 = mk<C>(fm * a0.x + f2 * a2.x + f0 * a3.x + f1 * a3.y, fm * a0.y + f2 * a2.y + f0 * a3.y - f1 * a3.x);
+                        const C h1 = mk<C>(fm * a1.x + f0 * a2.x - f1 * a2.y - f2 * a3.x, fm * a1.y + f0 * a2.y + f1 * a2.x - f2 * a3.y);
+                        const C h2 = mk<C>(f2 * a0.x + f0 * a1.x + f1 * a1.y - fm * a2.x, f2 * a0.y + f0 * a1.y - f1 * a1.x - fm * a2.y);
+                        const C h3 = mk<C>(f0 * a0.x - f1 * a0.y - f2 * a1.x - fm * a3.x, f0 * a0.y + f1 * a0.x - f2 * a1.y - fm * a3.y);
+                        y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
+                        y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
+                        y[2][i] = mk<C>(fc * a2.x + h2.y, fc * a2.y - h2.x);
+                        y[3][i] = mk<C>(fc * a3.x + h3.y, fc * a3.y - h3.x);
+                    }
+                }
+#pragma unroll
+                for (int c2 = 0; c2 < CC; ++c2)
+#pragma unroll
+                    for (int i = 0; i < PP; ++i) sm[(c2 * TL + t) * a.pitch + padp(u * 16 + c * PP + i)] = y[c2][i];
+                __syncthreads();
+#pragma unroll
+                for (int q = 0; q < 16; ++q) x[q] = sl[padp(u * 16 + q)];
+            }
+        }
+
+        if (a.do_dit) DitChain<T, N, LAST, -SIGN>::run(x, u, tw, sl);
+
+        if (a.post_v) {
+            if (rep + 1 < a.nrep) natural_v(a.post_v, n, n + 1, true);
+            else natural_v(a.post_v, n, n, false);
+        }
+    }
+
+    if (!a.do_dit && a.unpermute) {
+        // registers hold frequency revB[u] + U q at position 16 u + q: scatter to natural order
+        const int rb = a.revB[u];
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 16; ++q) sl[padp(rb + q * U)] = x[q];
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 16; ++q) x[q] = sl[padp(u + q * U)];
+    }
+    if (a.do_dit || a.unpermute) {
+#pragma unroll
+        for (int q = 0; q < 16; ++q) gp[(long long)(u + q * U) * estep] = x[q];
+    } else {
+#pragma unroll
+        for (int q = 0; q < 16; ++q) gp[(long long)(u * 16 + q) * estep] = x[q];
+    }
+}
+
+// host-side launcher, explicitly instantiated per (T, N) in sso_inst_*.cu
+template <typename T, int N, bool STRIDED, int PW, int SIGN>
+cudaError_t launch_pass(const PassArgs &a, unsigned grid, unsigned threads, size_t smem, cudaStream_t st);
+
+}  // namespace sso
