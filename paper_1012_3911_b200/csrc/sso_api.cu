@@ -305,22 +305,41 @@ int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double
                 revBinv[f] = p / 16;
             }
         }
-        // twiddles exp(-2 pi i t/n), evaluated in long double and rounded once to the plan's precision
+        // twiddles, evaluated in long double and rounded once to the plan's precision.  Stage i of the radix
+        // schedule (sub-transform length NP, radix R, NI = NP/R) stores w_NP^(l k) = exp(-2 pi i l k / NP) at
+        // [k-1][l], k = 1..R-1, l < NI; the last stage needs none.
+        std::vector<long double> twr, twi;
+        {
+            HostSched hs(n);
+            int NP = n;
+            for (int i = 0; i + 1 < hs.m; ++i) {
+                const int R = 1 << hs.lr[i], NI = NP / R;
+                for (int k = 1; k < R; ++k)
+                    for (int l = 0; l < NI; ++l) {
+                        const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)((long long)l * k % NP) / (long double)NP;
+                        twr.push_back(cosl(ang));
+                        twi.push_back(sinl(ang));
+                    }
+                NP = NI;
+            }
+            if (twr.empty()) {
+                twr.push_back(1.0L);
+                twi.push_back(0.0L);
+            }
+        }
         cudaError_t e;
         if (precision == SSO_C128) {
-            std::vector<double2> tw(n);
-            for (int t = 0; t < n; ++t) {
-                const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)t / (long double)n;
-                tw[t].x = (double)cosl(ang);
-                tw[t].y = (double)sinl(ang);
+            std::vector<double2> tw(twr.size());
+            for (size_t t = 0; t < twr.size(); ++t) {
+                tw[t].x = (double)twr[t];
+                tw[t].y = (double)twi[t];
             }
             e = upload(&A.tw, tw);
         } else {
-            std::vector<float2> tw(n);
-            for (int t = 0; t < n; ++t) {
-                const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)t / (long double)n;
-                tw[t].x = (float)cosl(ang);
-                tw[t].y = (float)sinl(ang);
+            std::vector<float2> tw(twr.size());
+            for (size_t t = 0; t < twr.size(); ++t) {
+                tw[t].x = (float)twr[t];
+                tw[t].y = (float)twi[t];
             }
             e = upload(&A.tw, tw);
         }

@@ -48,6 +48,24 @@ template <typename C> __device__ __forceinline__ C cmulc(C a, C b) {  // a * con
     return mk<C>(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
 }
 
+// psi is streamed: read once and written once per pass, so keep it out of L1 (the twiddle and phase tables
+// live there) but leave the L2 policy alone (the small configs stay L2-resident between passes)
+__device__ __forceinline__ double2 ld_stream(const double2 *p) {
+    double2 v;
+    asm volatile("ld.global.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float2 ld_stream(const float2 *p) {
+    float2 v;
+    asm volatile("ld.global.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+// ask L2 to fetch `bytes` (multiple of 16) starting at p; used for the potential table of a tile, which is
+// needed only after the first FFT
+__device__ __forceinline__ void prefetch_l2_bulk(const void *p, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 // ------------------------------------------------------------------------------------------
 // radix schedule: N = 2^LOG, last stage radix 16, the LOG-4 remaining bits in stages of <= 4 bits,
 // the first stage taking the remainder.
@@ -64,6 +82,12 @@ template <int N> struct Sched {
         int n = N;
         for (int j = 0; j < i; ++j) n >>= lr(j);
         return n;
+    }
+    // offset of stage i's twiddle block: stage j < M-1 stores (R_j - 1) * N_j entries, [k-1][l], l contiguous
+    __host__ __device__ static constexpr int twoff(int i) {
+        int o = 0;
+        for (int j = 0; j < i; ++j) o += ((1 << lr(j)) - 1) * (nprev(j) >> lr(j));
+        return o;
     }
 };
 
@@ -152,14 +176,15 @@ template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void di
 #pragma unroll
     for (int s = 0; s < S; ++s) dft_reg<R, S, SIGN>(&x[s]);
     if constexpr (NP > R) {
-        constexpr int TS = N / NP;
-        const int lp = u % Mi;
+        // twiddle w_NP^(l k) sits at [k-1][l] of this stage's block: consecutive threads (consecutive l') read
+        // consecutive entries
+        constexpr int NI = NP / R;
+        const C *__restrict__ tws = tw + Sched<N>::twoff(I) + (u % Mi);
 #pragma unroll
         for (int s = 0; s < S; ++s) {
-            const int l = s * Mi + lp;
 #pragma unroll
             for (int k = 1; k < R; ++k) {
-                const C w = __ldg(&tw[l * k * TS]);
+                const C w = __ldg(&tws[(k - 1) * NI + s * Mi]);
                 x[k * S + s] = SIGN < 0 ? cmul(x[k * S + s], w) : cmulc(x[k * S + s], w);
             }
         }
@@ -174,14 +199,15 @@ template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void di
     constexpr int Mi = NP / 16;
     constexpr int S = 16 / R;
     if constexpr (NP > R) {
-        constexpr int TS = N / NP;
-        const int lp = u % Mi;
+        // twiddle w_NP^(l k) sits at [k-1][l] of this stage's block: consecutive threads (consecutive l') read
+        // consecutive entries
+        constexpr int NI = NP / R;
+        const C *__restrict__ tws = tw + Sched<N>::twoff(I) + (u % Mi);
 #pragma unroll
         for (int s = 0; s < S; ++s) {
-            const int l = s * Mi + lp;
 #pragma unroll
             for (int k = 1; k < R; ++k) {
-                const C w = __ldg(&tw[l * k * TS]);
+                const C w = __ldg(&tws[(k - 1) * NI + s * Mi]);
                 x[k * S + s] = SIGN < 0 ? cmul(x[k * S + s], w) : cmulc(x[k * S + s], w);
             }
         }
@@ -307,10 +333,16 @@ __global__ void __launch_bounds__(512) pass_kernel(const PassArgs a) {
     C x[16];
     if (a.do_dif) {
 #pragma unroll
-        for (int q = 0; q < 16; ++q) x[q] = gp[(long long)(u + q * U) * estep];
+        for (int q = 0; q < 16; ++q) x[q] = ld_stream(&gp[(long long)(u + q * U) * estep]);
     } else {
 #pragma unroll
-        for (int q = 0; q < 16; ++q) x[q] = gp[(long long)(u * 16 + q) * estep];
+        for (int q = 0; q < 16; ++q) x[q] = ld_stream(&gp[(long long)(u * 16 + q) * estep]);
+    }
+    if constexpr (PW == PW_V) {
+        if (a.mid_on && u == 0) {
+            const size_t esz = a.vrep == VREP_TABLE ? sizeof(C) : sizeof(double);
+            prefetch_l2_bulk(reinterpret_cast<const char *>(a.vtab) + (size_t)line * N * esz, (unsigned)(N * esz));
+        }
     }
 
     // angle of the homogeneous-field phase contributed by the non-line axes of this line:
