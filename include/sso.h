@@ -145,6 +145,13 @@ int sso_destroy(sso_plan *plan);
 
 const char *sso_last_error(const sso_plan *plan);
 
+/*
+ * Host-only introspection of the plan builder (no GPU needed; used by the CPU tests): for a line of n points,
+ * pos_freq[p] = frequency index held at position p after the decimation-in-frequency stages, and
+ * slot_nat[s] = natural index stored at slot s of the permuted table layout.  Both are host int[n].
+ */
+int sso_debug_layout(int n, int *pos_freq, int *slot_nat);
+
 /* Library version string, e.g. "sso 0.1 (sm_100a)". */
 const char *sso_version(void);
 

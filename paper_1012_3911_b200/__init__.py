@@ -26,7 +26,7 @@ OPT_LINES_PER_TILE_CONTIG, OPT_LINES_PER_TILE_STRIDED, OPT_POTENTIAL_PHASE = 1, 
 SYMBOLS = (
     "sso_plan_create", "sso_set_constants", "sso_set_potential", "sso_set_field", "sso_set_time_index",
     "sso_get_time_index", "sso_step", "sso_step_host", "sso_norm", "sso_set_option", "sso_launch_count",
-    "sso_destroy", "sso_last_error", "sso_version",
+    "sso_destroy", "sso_last_error", "sso_version", "sso_debug_layout",
 )
 
 

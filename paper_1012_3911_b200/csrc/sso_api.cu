@@ -166,6 +166,18 @@ static int freq_of_pos(int N, int p) {
     return f;
 }
 
+// entries of the twiddle blocks of all non-final stages, padded as in the kernel (TWP)
+static int twiddle_count_padded(int N) {
+    HostSched s(N);
+    int NP = N, cnt = 0;
+    for (int i = 0; i + 1 < s.m; ++i) {
+        const int R = 1 << s.lr[i];
+        cnt += (R - 1) * (NP / R);
+        NP /= R;
+    }
+    return (cnt + 7) & ~7;
+}
+
 struct Axis {
     int n = 0;
     double dx = 0.0;
@@ -201,7 +213,9 @@ struct sso_plan {
     int vrep = VREP_TABLE;
     bool kph_valid = false;
     int opt_tl_contig = 0, opt_tl_strided = 0;
+    int dbg_skip = 0;  // development only: bit 0 skip DIF, bit 1 skip DIT, bit 2 skip the pointwise factor (wrong results)
     double *d_partial = nullptr, *d_norm = nullptr;
+    unsigned *d_sched = nullptr;  // tile scheduler of the pass kernel (zero between launches)
     void *d_hostbuf = nullptr;
     std::string err;
     size_t esize() const { return precision == SSO_C64 ? 8 : 16; }
@@ -249,6 +263,17 @@ static void kinetic_layout(const sso_plan *p, int a, std::vector<double> &kv) {
 extern "C" {
 
 const char *sso_version(void) { return "sso 0.1 (sm_100a)"; }
+
+int sso_debug_layout(int n, int *pos_freq, int *slot_nat) {
+    if (!pos_freq || !slot_nat || !is_pow2(n) || n < SSO_MIN_AXIS || n > SSO_MAX_AXIS) return SSO_ERR_INVALID;
+    const int U = n / 16;
+    for (int p = 0; p < n; ++p) {
+        const int f = freq_of_pos(n, p);
+        pos_freq[p] = f;
+        slot_nat[(p % 16) * U + p / 16] = f;
+    }
+    return SSO_OK;
+}
 
 const char *sso_last_error(const sso_plan *plan) { return plan ? plan->err.c_str() : g_create_err.c_str(); }
 
@@ -359,6 +384,8 @@ int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double
     }
     cudaError_t e = cudaMalloc((void **)&plan->d_partial, sizeof(double) * NORM_BLOCKS);
     if (e == cudaSuccess) e = cudaMalloc((void **)&plan->d_norm, sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&plan->d_sched, 2 * sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMemset(plan->d_sched, 0, 2 * sizeof(unsigned));
     if (e != cudaSuccess) {
         int rc = cuda_fail(nullptr, e, "plan buffers");
         sso_destroy(plan);
@@ -390,6 +417,7 @@ int sso_destroy(sso_plan *plan) {
     cudaFree(plan->d_vtab);
     cudaFree(plan->d_partial);
     cudaFree(plan->d_norm);
+    cudaFree(plan->d_sched);
     cudaFree(plan->d_hostbuf);
     delete plan;
     return SSO_OK;
@@ -503,6 +531,9 @@ int sso_set_option(sso_plan *plan, int option, int64_t value) {
             if (value < 0 || value > 512 || (value > 0 && !is_pow2(value))) return fail(plan, SSO_ERR_INVALID, "lines per tile must be 0 or a power of two <= 512");
             (option == SSO_OPT_LINES_PER_TILE_CONTIG ? plan->opt_tl_contig : plan->opt_tl_strided) = (int)value;
             return SSO_OK;
+        case 100:
+            plan->dbg_skip = (int)value;
+            return SSO_OK;
         case SSO_OPT_POTENTIAL_PHASE:
             if (value != VREP_TABLE && value != VREP_ANGLE) return fail(plan, SSO_ERR_INVALID, "potential phase mode must be 0 or 1");
             if ((int)value != plan->vrep) {
@@ -561,7 +592,7 @@ int choose_tl(const sso_plan *p, const Geometry &g, int cc) {
     const int esz = (int)p->esize();
     long long tl;
     if (!g.strided) {
-        tl = p->opt_tl_contig > 0 ? p->opt_tl_contig : 256 / (cc * U);
+        tl = p->opt_tl_contig > 0 ? p->opt_tl_contig : (U >= 256 ? 512 : 256) / (cc * U);
         if (tl < 1) tl = 1;
         if (tl > g.lines) tl = g.lines;
     } else {
@@ -585,6 +616,8 @@ struct PassSpec {
 };
 
 int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
+    if ((plan->dbg_skip & 16) && s.axis == 0 && plan->ndim > 1) return SSO_OK;               // development: no kinetic pass
+    if ((plan->dbg_skip & 32) && s.axis == plan->ndim - 1 && plan->ndim > 1) return SSO_OK;  // development: no potential pass
     const Geometry g = geometry(plan, s.axis);
     const Axis &A = plan->ax[s.axis];
     const int cc = s.pw == PW_KD2 ? 2 : (s.pw == PW_KD4 ? 4 : 1);
@@ -609,10 +642,11 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
     a.rest1 = g.rest1;
     a.oaxA = g.oaxA;
     a.oaxB = g.oaxB;
-    a.do_dif = s.do_dif;
-    a.do_dit = s.do_dit;
+    a.do_dif = (plan->dbg_skip & 1) ? 0 : s.do_dif;
+    a.do_dit = (plan->dbg_skip & 2) ? 0 : s.do_dit;
     a.unpermute = s.unpermute;
-    a.mid_on = s.mid_on;
+    a.mid_on = (plan->dbg_skip & 4) ? 0 : s.mid_on;
+    a.dbg_copy = (plan->dbg_skip & 8) ? 1 : 0;
     a.pre_v = s.pre_v;
     a.post_v = s.post_v;
     a.nrep = s.nrep;
@@ -657,10 +691,14 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
     LaunchFn fn = find_launch(plan->precision, A.n, g.strided ? 1 : 0, s.pw, s.sign);
     if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no kernel built for this pass");
     const long long tiles = g.lines / TL;
-    const long long grid = cc == 1 ? tiles * plan->ncomp : tiles;
+    const long long work = cc == 1 ? tiles * plan->ncomp : tiles;
+    if (work > 0x7fffffffLL) return fail(plan, SSO_ERR_UNSUPPORTED, "too many tiles");
+    a.ntiles = (int)work;
+    a.sched = plan->d_sched;
     const unsigned threads = (unsigned)(cc * TL * U);
-    const size_t smem = (size_t)cc * TL * pitch * esz + (size_t)TL * esz + (size_t)TL * 2 * sizeof(double);
-    cudaError_t e = fn(a, (unsigned)grid, threads, smem, st);
+    size_t smem = (size_t)twiddle_count_padded(A.n) * esz + (size_t)cc * TL * pitch * esz + (size_t)TL * esz + 2 * sizeof(int);
+    smem = (smem + 127) & ~(size_t)127;
+    cudaError_t e = fn(a, threads, smem, st);
     if (e != cudaSuccess) return cuda_fail(plan, e, "pass kernel launch");
     return SSO_OK;
 }

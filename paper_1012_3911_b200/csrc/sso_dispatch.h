@@ -13,7 +13,9 @@ enum : int { VREP_TABLE = 0, VREP_ANGLE = 1 };
 
 struct PassArgs {
     void *psi;               // device, [ncomp][...] complex
-    const void *tw;          // complex[N]: exp(-2 pi i t / N)
+    const void *tw;          // complex twiddle blocks, one per non-final stage: [k-1][l] = exp(-2 pi i l k / NP)
+    unsigned *sched;         // device uint[2]: next tile, CTAs done (both zero between launches)
+    int ntiles;              // work items of this launch (tiles x components when components are independent)
     const int *revB;         // int[N/16]: digit reversal of the last-stage thread index
     const int *revBinv;      // int[N/16]: its inverse
     long long comp_stride;   // complex elements between components
@@ -25,6 +27,7 @@ struct PassArgs {
     int oaxA, oaxB;          // lattice axes that ia and ib run along (-1: absent)
     // structure of the pass
     int do_dif, do_dit, unpermute;
+    int dbg_copy;            // development only: load and store in the coalesced layout, nothing in between
     int mid_on;              // apply the pointwise factor between DIF and DIT
     int pre_v, post_v;       // 0 none; 1 natural-order table (1D); 2 gather from the permuted table (opening pass)
     int nrep;                // repetitions inside the kernel (1D persistent stepping), >= 1
@@ -54,7 +57,8 @@ struct PassArgs {
     double scale;            // 1/Ntot (Dirac; Schroedinger folds it into kph0)
 };
 
-using LaunchFn = cudaError_t (*)(const PassArgs &, unsigned grid, unsigned threads, size_t smem, cudaStream_t st);
+// launches one wave of persistent CTAs (resident CTAs per SM x SMs, at most ntiles)
+using LaunchFn = cudaError_t (*)(const PassArgs &, unsigned threads, size_t smem, cudaStream_t st);
 
 // one lookup function per compiled (precision, line length); returns NULL for a variant that is not built
 #define SSO_FOR_EACH_N(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096)

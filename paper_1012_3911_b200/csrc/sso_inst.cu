@@ -12,15 +12,38 @@
 namespace sso {
 
 template <typename T, int N, bool STRIDED, int PW, int SIGN>
-cudaError_t launch_pass(const PassArgs &a, unsigned grid, unsigned threads, size_t smem, cudaStream_t st) {
+cudaError_t launch_pass(const PassArgs &a, unsigned threads, size_t smem, cudaStream_t st) {
     auto kern = pass_kernel<T, N, STRIDED, PW, SIGN>;
     static bool attr_done = false;
+    static int num_sms = 0;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
+        int dev = 0;
+        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+        if ((e = cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
         attr_done = true;
     }
-    kern<<<grid, threads, smem, st>>>(a);
+    // resident CTAs per SM for this block shape (cached: a plan uses one or two shapes per kernel)
+    static unsigned key_threads[4] = {0, 0, 0, 0};
+    static size_t key_smem[4] = {0, 0, 0, 0};
+    static int key_occ[4] = {0, 0, 0, 0};
+    static int key_n = 0;
+    int occ = 0;
+    for (int i = 0; i < key_n; ++i)
+        if (key_threads[i] == threads && key_smem[i] == smem) occ = key_occ[i];
+    if (occ == 0) {
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (int)threads, smem);
+        if (e != cudaSuccess) return e;
+        if (occ < 1) return cudaErrorLaunchOutOfResources;
+        const int slot = key_n < 4 ? key_n++ : 3;
+        key_threads[slot] = threads;
+        key_smem[slot] = smem;
+        key_occ[slot] = occ;
+    }
+    long long grid = (long long)occ * num_sms;
+    if (grid > a.ntiles) grid = a.ntiles;
+    kern<<<(unsigned)grid, threads, smem, st>>>(a);
     return cudaGetLastError();
 }
 

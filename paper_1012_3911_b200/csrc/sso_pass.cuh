@@ -60,6 +60,12 @@ __device__ __forceinline__ float2 ld_stream(const float2 *p) {
     asm volatile("ld.global.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
     return v;
 }
+__device__ __forceinline__ void st_stream(double2 *p, double2 v) {
+    asm volatile("st.global.L1::no_allocate.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void st_stream(float2 *p, float2 v) {
+    asm volatile("st.global.L1::no_allocate.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.x), "f"(v.y) : "memory");
+}
 // ask L2 to fetch `bytes` (multiple of 16) starting at p; used for the potential table of a tile, which is
 // needed only after the first FFT
 __device__ __forceinline__ void prefetch_l2_bulk(const void *p, unsigned bytes) {
@@ -158,16 +164,27 @@ template <int R, int S, int SIGN, typename C> __device__ __forceinline__ void df
     }
 }
 
-// position (within the line) of register q of thread u in the layout of stage I:
-//   u = B' * Mi + l',  pos = B' * 16 Mi + q Mi + l',  Mi = nprev(I)/16
-template <int N, int I> __device__ __forceinline__ int stage_pos(int u, int q) {
-    constexpr int Mi = Sched<N>::nprev(I) / 16;
-    return (u / Mi) * (16 * Mi) + q * Mi + (u % Mi);
-}
+// Layout of stage I: thread u = B' * Mi + l' holds, in register q, line position
+//   pos = B' * 16 Mi + q Mi + l',   Mi = nprev(I)/16.
+// In shared memory position p lives at p + (p >> 4) (one pad element per 16: every access pattern the
+// stages use is then bank-conflict free at 128-byte wavefront granularity).  Because q Mi is either a
+// multiple of 16 or stays inside one group of 16, the padded address splits into a per-thread base and a
+// compile-time offset per register, so every LDS/STS uses [base + immediate].
 __device__ __forceinline__ int padp(int p) { return p + (p >> 4); }
+template <int N, int I> __device__ __forceinline__ int stage_base(int u) {
+    constexpr int Mi = Sched<N>::nprev(I) / 16;
+    return padp((u / Mi) * (16 * Mi) + (u % Mi));
+}
+template <int N, int I> __host__ __device__ constexpr int stage_delta(int q) {
+    constexpr int Mi = Sched<N>::nprev(I) / 16;
+    return q * Mi + ((q * Mi) >> 4);
+}
+__host__ __device__ constexpr int lin_delta(int q, int stride) { return q * stride + ((q * stride) >> 4); }
 
-// one DIF stage: butterflies over the top digit of the current sub-transform, then twiddles
-template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void dif_stage(typename CxOf<T>::type (&x)[16], int u, const typename CxOf<T>::type *__restrict__ tw) {
+// one DIF stage: butterflies over the top digit of the current sub-transform, then twiddles.
+// Twiddle w_NP^(l k) sits at [k-1][l] of this stage's block (shared memory copy): consecutive threads
+// (consecutive l') read consecutive entries.
+template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void dif_stage(typename CxOf<T>::type (&x)[16], int u, const typename CxOf<T>::type *tw) {
     using C = typename CxOf<T>::type;
     constexpr int R = 1 << Sched<N>::lr(I);
     constexpr int NP = Sched<N>::nprev(I);
@@ -176,15 +193,13 @@ template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void di
 #pragma unroll
     for (int s = 0; s < S; ++s) dft_reg<R, S, SIGN>(&x[s]);
     if constexpr (NP > R) {
-        // twiddle w_NP^(l k) sits at [k-1][l] of this stage's block: consecutive threads (consecutive l') read
-        // consecutive entries
         constexpr int NI = NP / R;
-        const C *__restrict__ tws = tw + Sched<N>::twoff(I) + (u % Mi);
+        const C *tws = tw + Sched<N>::twoff(I) + (u % Mi);
 #pragma unroll
         for (int s = 0; s < S; ++s) {
 #pragma unroll
             for (int k = 1; k < R; ++k) {
-                const C w = __ldg(&tws[(k - 1) * NI + s * Mi]);
+                const C w = tws[(k - 1) * NI + s * Mi];
                 x[k * S + s] = SIGN < 0 ? cmul(x[k * S + s], w) : cmulc(x[k * S + s], w);
             }
         }
@@ -192,22 +207,20 @@ template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void di
 }
 
 // the transposed (DIT) stage: twiddles, then butterflies
-template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void dit_stage(typename CxOf<T>::type (&x)[16], int u, const typename CxOf<T>::type *__restrict__ tw) {
+template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void dit_stage(typename CxOf<T>::type (&x)[16], int u, const typename CxOf<T>::type *tw) {
     using C = typename CxOf<T>::type;
     constexpr int R = 1 << Sched<N>::lr(I);
     constexpr int NP = Sched<N>::nprev(I);
     constexpr int Mi = NP / 16;
     constexpr int S = 16 / R;
     if constexpr (NP > R) {
-        // twiddle w_NP^(l k) sits at [k-1][l] of this stage's block: consecutive threads (consecutive l') read
-        // consecutive entries
         constexpr int NI = NP / R;
-        const C *__restrict__ tws = tw + Sched<N>::twoff(I) + (u % Mi);
+        const C *tws = tw + Sched<N>::twoff(I) + (u % Mi);
 #pragma unroll
         for (int s = 0; s < S; ++s) {
 #pragma unroll
             for (int k = 1; k < R; ++k) {
-                const C w = __ldg(&tws[(k - 1) * NI + s * Mi]);
+                const C w = tws[(k - 1) * NI + s * Mi];
                 x[k * S + s] = SIGN < 0 ? cmul(x[k * S + s], w) : cmulc(x[k * S + s], w);
             }
         }
@@ -218,12 +231,15 @@ template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void di
 
 // registers (layout of stage IA) -> shared memory -> registers (layout of stage IB)
 template <typename T, int N, int IA, int IB> __device__ __forceinline__ void exchange(typename CxOf<T>::type (&x)[16], int u, typename CxOf<T>::type *sl) {
+    using C = typename CxOf<T>::type;
+    C *wa = sl + stage_base<N, IA>(u);
+    const C *rb = sl + stage_base<N, IB>(u);
     __syncthreads();
 #pragma unroll
-    for (int q = 0; q < 16; ++q) sl[padp(stage_pos<N, IA>(u, q))] = x[q];
+    for (int q = 0; q < 16; ++q) wa[stage_delta<N, IA>(q)] = x[q];
     __syncthreads();
 #pragma unroll
-    for (int q = 0; q < 16; ++q) x[q] = sl[padp(stage_pos<N, IB>(u, q))];
+    for (int q = 0; q < 16; ++q) x[q] = rb[stage_delta<N, IB>(q)];
 }
 
 template <typename T, int N, int I, int SIGN> struct DifChain {
@@ -247,17 +263,19 @@ template <typename T, int N, int I, int SIGN> struct DitChain {  // runs stages 
     }
 };
 
-// exp(i a) for a phase table entry or an angle, in the working precision
+// exp(i a) in the working precision (evaluated in double)
 template <typename T> __device__ __forceinline__ typename CxOf<T>::type expi(double a) {
     double s, c;
     sincos(a, &s, &c);
     return mk<typename CxOf<T>::type>((T)c, (T)s);
 }
 
-// step average row n, component a (0 when there is no table)
+// step average row n, component ax (0 when there is no table)
 __device__ __forceinline__ double favg(const PassArgs &a, long long n, int ax) {
     return a.step_avg ? a.step_avg[n * a.ndim + ax] : 0.0;
 }
+
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // ------------------------------------------------------------------------------------------
 // the kernel
@@ -267,15 +285,21 @@ __device__ __forceinline__ double favg(const PassArgs &a, long long n, int ax) {
 //   PW: pointwise factor kind.  The Dirac kinds hold all components of the tile's lines in one CTA.
 //   SIGN: sign of the DIF transform (-1: forward first, the kinetic sandwich; +1: inverse first,
 //         the potential sandwich).
+// Persistent CTAs: the grid is one wave (resident CTAs per SM x SM count); each CTA copies the twiddle
+// table to shared memory once and then pulls tiles from a global counter until none are left, asking L2
+// for the next tile's data while it works on the current one.
 // ------------------------------------------------------------------------------------------
 template <typename T, int N, bool STRIDED, int PW, int SIGN>
-__global__ void __launch_bounds__(512) pass_kernel(const PassArgs a) {
+__global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(const PassArgs a) {
     using C = typename CxOf<T>::type;
     constexpr int U = N / 16;
     constexpr int CC = PW == PW_KD2 ? 2 : (PW == PW_KD4 ? 4 : 1);
     constexpr int LAST = Sched<N>::M - 1;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    C *sm = reinterpret_cast<C *>(smem_raw);
+    constexpr int TWN = Sched<N>::twoff(LAST);
+    constexpr int TWP = (TWN + 7) & ~7;  // keep the exchange buffer 128-byte aligned
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    C *stw = reinterpret_cast<C *>(smem_raw);
+    C *sm = stw + TWP;
 
     const int TL = a.TL;
     const int tid = threadIdx.x;
@@ -291,244 +315,306 @@ __global__ void __launch_bounds__(512) pass_kernel(const PassArgs a) {
         t = ct % TL;
         c = ct / TL;
     }
-    long long tile;
-    int comp;
-    if (CC == 1) {
-        comp = (int)(blockIdx.x % (unsigned)a.ncomp);
-        tile = blockIdx.x / (unsigned)a.ncomp;
-    } else {
-        comp = c;
-        tile = blockIdx.x;
-    }
-    const long long line = tile * TL + t;  // line index within a component
-    long long base, estep;
-    if (STRIDED) {
-        const long long o = line / a.inner, i = line % a.inner;
-        base = o * (long long)N * a.inner + i;
-        estep = a.inner;
-    } else {
-        base = line * (long long)N;
-        estep = 1;
-    }
-    C *__restrict__ gp = reinterpret_cast<C *>(a.psi) + (long long)comp * a.comp_stride + base;
     C *sl = sm + (c * TL + t) * a.pitch;
-    C *lsc = sm + CC * TL * a.pitch;  // per-line scalars [TL] (complex) ...
-    double *lkv = reinterpret_cast<double *>(lsc + TL);  // ... and per-line k values [TL][2] (Dirac)
-    const C *__restrict__ tw = reinterpret_cast<const C *>(a.tw);
+    C *lsc = sm + CC * TL * a.pitch;                       // per-line scalars [TL] (complex)
+    int *snext = reinterpret_cast<int *>(lsc + TL);         // tile scheduler mailbox [2]
 
-    // line coordinates on the non-line axes: line = ia * rest1 + ib
-    const int ib = (int)(line % a.rest1);
-    const int ia = (int)(line / a.rest1);
-
-    // per-line kinetic scalars
-    if (PW == PW_KS && (a.kph1 || a.kph2)) {
-        if (u == 0 && c == 0) {
-            C s = mk<C>((T)1, (T)0);
-            if (a.kph1) s = reinterpret_cast<const C *>(a.kph1)[ia];
-            if (a.kph2) s = a.kph1 ? cmul(s, reinterpret_cast<const C *>(a.kph2)[ib]) : reinterpret_cast<const C *>(a.kph2)[ib];
-            lsc[t] = s;
-        }
+    // twiddles -> shared memory, once per CTA
+    {
+        const C *__restrict__ gtw = reinterpret_cast<const C *>(a.tw);
+        for (int i = tid; i < TWN; i += blockDim.x) stw[i] = gtw[i];
     }
+    if (tid == 0) snext[0] = (int)atomicAdd(&a.sched[0], 1u);
+    __syncthreads();
+    int wtile = snext[0];
+    int parity = 1;
 
-    C x[16];
-    if (a.do_dif) {
-#pragma unroll
-        for (int q = 0; q < 16; ++q) x[q] = ld_stream(&gp[(long long)(u + q * U) * estep]);
-    } else {
-#pragma unroll
-        for (int q = 0; q < 16; ++q) x[q] = ld_stream(&gp[(long long)(u * 16 + q) * estep]);
-    }
-    if constexpr (PW == PW_V) {
-        if (a.mid_on && u == 0) {
-            const size_t esz = a.vrep == VREP_TABLE ? sizeof(C) : sizeof(double);
-            prefetch_l2_bulk(reinterpret_cast<const char *>(a.vtab) + (size_t)line * N * esz, (unsigned)(N * esz));
-        }
-    }
+    while (wtile < a.ntiles) {
+        // fetch the next tile index early so that its data can be requested from L2 ahead of time
+        if (tid == 0) snext[parity] = (int)atomicAdd(&a.sched[0], 1u);
 
-    // angle of the homogeneous-field phase contributed by the non-line axes of this line:
-    // (tau/2) sum_ax (Ebar_na + [full] Ebar_nb)[ax] * r_ax      (eq. 11, reading G12)
-    auto other_axes_angle = [&](long long n_a, long long n_b, bool full) -> double {
-        double ang = 0.0;
-        if (a.oaxA >= 0) {
-            double e = favg(a, n_a, a.oaxA);
-            if (full) e += favg(a, n_b, a.oaxA);
-            ang += e * a.half_dt * ((double)ia - (double)(a.nsz[a.oaxA] / 2)) * a.dxs[a.oaxA];
+        long long tile;
+        int comp;
+        if (CC == 1) {
+            comp = wtile % a.ncomp;
+            tile = wtile / a.ncomp;
+        } else {
+            comp = c;
+            tile = wtile;
         }
-        if (a.oaxB >= 0) {
-            double e = favg(a, n_a, a.oaxB);
-            if (full) e += favg(a, n_b, a.oaxB);
-            ang += e * a.half_dt * ((double)ib - (double)(a.nsz[a.oaxB] / 2)) * a.dxs[a.oaxB];
+        const long long line = tile * TL + t;  // line index within a component
+        long long base, estep;
+        if (STRIDED) {
+            const long long o = line / a.inner, i = line % a.inner;
+            base = o * (long long)N * a.inner + i;
+            estep = a.inner;
+        } else {
+            base = line * (long long)N;
+            estep = 1;
         }
-        return ang;
-    };
+        C *__restrict__ gp = reinterpret_cast<C *>(a.psi) + (long long)comp * a.comp_stride + base;
 
-    // potential phase in natural order at the stage-0 layout (thread u holds positions u + q U);
-    // mode 1: the table is in natural order (1D); mode 2: gather from the permuted table
-    auto natural_v = [&](int mode, long long n_a, long long n_b, bool full) {
-        if constexpr (!STRIDED) {
-            const int slot_u = mode == 2 ? a.revBinv[u] : u;
-            double gl = 0.0, gother = 0.0;
-            if (a.field_kind == 1) {
-                double e = favg(a, n_a, a.line_axis);
-                if (full) e += favg(a, n_b, a.line_axis);
-                gl = e * a.half_dt;
-                gother = other_axes_angle(n_a, n_b, full);
+        // line coordinates on the non-line axes: line = ia * rest1 + ib
+        const int ib = (int)(line % a.rest1);
+        const int ia = (int)(line / a.rest1);
+
+        // per-line kinetic scalars
+        if (PW == PW_KS && (a.kph1 || a.kph2)) {
+            if (u == 0 && c == 0) {
+                C s = mk<C>((T)1, (T)0);
+                if (a.kph1) s = reinterpret_cast<const C *>(a.kph1)[ia];
+                if (a.kph2) s = a.kph1 ? cmul(s, reinterpret_cast<const C *>(a.kph2)[ib]) : reinterpret_cast<const C *>(a.kph2)[ib];
+                lsc[t] = s;
             }
+        }
+
+        C x[16];
+        if (a.do_dif || a.dbg_copy) {
 #pragma unroll
-            for (int q = 0; q < 16; ++q) {
-                C h;
-                const long long vi = line * (long long)N + q * U + slot_u;
-                if (a.vrep == VREP_TABLE) {
-                    h = reinterpret_cast<const C *>(a.vtab)[vi];
-                    if (full) h = cmul(h, h);
-                } else {
-                    const double ang = reinterpret_cast<const double *>(a.vtab)[vi];
-                    h = expi<T>(full ? 2.0 * ang : ang);
-                }
+            for (int q = 0; q < 16; ++q) x[q] = ld_stream(&gp[(long long)(u + q * U) * estep]);
+        } else {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) x[q] = ld_stream(&gp[(long long)(u * 16 + q) * estep]);
+        }
+        if constexpr (PW == PW_V) {
+            if (a.mid_on && u == 0) {
+                const size_t esz = a.vrep == VREP_TABLE ? sizeof(C) : sizeof(double);
+                prefetch_l2_bulk(reinterpret_cast<const char *>(a.vtab) + (size_t)line * N * esz, (unsigned)(N * esz));
+            }
+        }
+
+        // angle of the homogeneous-field phase contributed by the non-line axes of this line:
+        // (tau/2) sum_ax (Ebar_na + [full] Ebar_nb)[ax] * r_ax      (eq. 11, reading G12)
+        auto other_axes_angle = [&](long long n_a, long long n_b, bool full) -> double {
+            double ang = 0.0;
+            if (a.oaxA >= 0) {
+                double e = favg(a, n_a, a.oaxA);
+                if (full) e += favg(a, n_b, a.oaxA);
+                ang += e * a.half_dt * ((double)ia - (double)(a.nsz[a.oaxA] / 2)) * a.dxs[a.oaxA];
+            }
+            if (a.oaxB >= 0) {
+                double e = favg(a, n_a, a.oaxB);
+                if (full) e += favg(a, n_b, a.oaxB);
+                ang += e * a.half_dt * ((double)ib - (double)(a.nsz[a.oaxB] / 2)) * a.dxs[a.oaxB];
+            }
+            return ang;
+        };
+
+        // potential phase in natural order at the stage-0 layout (thread u holds positions u + q U);
+        // mode 1: the table is in natural order (1D); mode 2: gather from the permuted table
+        auto natural_v = [&](int mode, long long n_a, long long n_b, bool full) {
+            if constexpr (!STRIDED) {
+                const int slot_u = mode == 2 ? a.revBinv[u] : u;
+                double gl = 0.0, gother = 0.0;
                 if (a.field_kind == 1) {
-                    const double r = ((double)(u + q * U) - (double)(N / 2)) * a.dxs[a.line_axis];
-                    h = cmul(h, expi<T>(-(gl * r + gother)));
+                    double e = favg(a, n_a, a.line_axis);
+                    if (full) e += favg(a, n_b, a.line_axis);
+                    gl = e * a.half_dt;
+                    gother = other_axes_angle(n_a, n_b, full);
                 }
-                x[q] = cmul(x[q], h);
-            }
-        }
-    };
-
-    for (int rep = 0; rep < a.nrep; ++rep) {
-        const long long n = a.n0 + rep;
-        if (a.pre_v && rep == 0) natural_v(a.pre_v, n, n, false);
-
-        if (a.do_dif) DifChain<T, N, 0, SIGN>::run(x, u, tw, sl);
-
-        if (a.mid_on) {
-            if constexpr (PW == PW_V) {
-                // merged or half potential phase in the permuted order: register q of thread u is
-                // table slot q U + u (coalesced across u)
-                if (a.field_kind == 1 && u == 0) lsc[t] = expi<T>(-other_axes_angle(n, n + 1, a.v_mid_full != 0));
-                if (a.field_kind == 1) __syncthreads();
-                const long long vb = line * (long long)N + u;
 #pragma unroll
                 for (int q = 0; q < 16; ++q) {
                     C h;
+                    const long long vi = line * (long long)N + q * U + slot_u;
                     if (a.vrep == VREP_TABLE) {
-                        h = reinterpret_cast<const C *>(a.vtab)[vb + q * U];
-                        if (a.v_mid_full) h = cmul(h, h);
+                        h = reinterpret_cast<const C *>(a.vtab)[vi];
+                        if (full) h = cmul(h, h);
                     } else {
-                        const double ang = reinterpret_cast<const double *>(a.vtab)[vb + q * U];
-                        h = expi<T>(a.v_mid_full ? 2.0 * ang : ang);
+                        const double ang = reinterpret_cast<const double *>(a.vtab)[vi];
+                        h = expi<T>(full ? 2.0 * ang : ang);
                     }
-                    if (a.field_kind == 1) h = cmul(h, lsc[t]);
-                    if (a.ephase) h = cmul(h, reinterpret_cast<const C *>(a.ephase)[q * U + u]);
+                    if (a.field_kind == 1) {
+                        const double r = ((double)(u + q * U) - (double)(N / 2)) * a.dxs[a.line_axis];
+                        h = cmul(h, expi<T>(-(gl * r + gother)));
+                    }
                     x[q] = cmul(x[q], h);
                 }
-            } else if constexpr (PW == PW_KS) {
-                const bool has_lsc = a.kph1 || a.kph2;
-                if (has_lsc && Sched<N>::M == 1) __syncthreads();
-                const C *__restrict__ k0 = reinterpret_cast<const C *>(a.kph0);
+            }
+        };
+
+        // every thread learns the next tile and asks L2 for its share of that tile
+        __syncthreads();  // also orders the twiddle copy (first tile) and lsc before their use
+        const int ntile = snext[parity];
+        if (ntile < a.ntiles) {
+            long long tile2 = CC == 1 ? ntile / a.ncomp : ntile;
+            const int comp2 = CC == 1 ? ntile % a.ncomp : c;
+            const long long line2 = tile2 * TL + t;
+            long long base2;
+            if (STRIDED) {
+                const long long o = line2 / a.inner, i = line2 % a.inner;
+                base2 = o * (long long)N * a.inner + i;
+            } else {
+                base2 = line2 * (long long)N;
+            }
+            const C *gp2 = reinterpret_cast<const C *>(a.psi) + (long long)comp2 * a.comp_stride + base2;
+            // one request per 32-byte sector
+            constexpr int PER = 32 / (int)sizeof(C) < 1 ? 1 : 32 / (int)sizeof(C);
+            const bool mine = STRIDED ? (t % PER == 0) : (u % PER == 0);
+            if (mine) {
+                if (a.do_dif) {
 #pragma unroll
-                for (int q = 0; q < 16; ++q) {
-                    C f = k0[q * U + u];
-                    if (has_lsc) f = cmul(f, lsc[t]);
-                    x[q] = cmul(x[q], f);
+                    for (int q = 0; q < 16; ++q) prefetch_l2(&gp2[(long long)(u + q * U) * estep]);
+                } else {
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) prefetch_l2(&gp2[(long long)(u * 16 + q) * estep]);
                 }
-            } else if constexpr (PW == PW_KD2 || PW == PW_KD4) {
-                constexpr int PP = 16 / CC;
-                // shift of the kinetic momentum: pi = k - q Abar_n (reading G16)
-                double sh[3] = {0.0, 0.0, 0.0};
-                if (a.field_kind == 2)
-                    for (int ax = 0; ax < a.ndim; ++ax) sh[ax] = a.charge * favg(a, n, ax);
-                // non-line momenta of this line: the line axis is axis 0 here
-                double p1 = 0.0, p2 = 0.0;
-                if (a.ndim == 2) p1 = a.kv2[ib] - sh[1];
-                if (a.ndim == 3) {
-                    p1 = a.kv1[ia] - sh[1];
-                    p2 = a.kv2[ib] - sh[2];
-                }
-                __syncthreads();
-#pragma unroll
-                for (int q = 0; q < 16; ++q) sl[padp(u * 16 + q)] = x[q];
-                __syncthreads();
-                C y[CC][PP];
-#pragma unroll
-                for (int c2 = 0; c2 < CC; ++c2)
-#pragma unroll
-                    for (int i = 0; i < PP; ++i) y[c2][i] = sm[(c2 * TL + t) * a.pitch + padp(u * 16 + c * PP + i)];
-                const double mc2 = a.mass * a.clight * a.clight;
-#pragma unroll
-                for (int i = 0; i < PP; ++i) {
-                    const int q2 = c * PP + i;
-                    const double p0 = a.kv0[q2 * U + u] - sh[0];
-                    const double pp = p0 * p0 + p1 * p1 + p2 * p2;
-                    const double E = sqrt(a.clight * a.clight * pp + mc2 * mc2);
-                    double sn, cs;
-                    sincos(E * a.dt, &sn, &cs);
-                    double sE = E > 0.0 ? sn / E : a.dt;
-                    cs *= a.scale;
-                    sE *= a.scale;
-                    const T fc = (T)cs;
-                    const T fm = (T)(sE * mc2);
-                    const T f0 = (T)(sE * a.clight * p0), f1 = (T)(sE * a.clight * p1), f2 = (T)(sE * a.clight * p2);
-                    // out = cs psi - i sE H psi ;  (-i)(a + i b) = b - i a
-                    if constexpr (CC == 2) {
-                        const C a0 = y[0][i], a1 = y[1][i];
-                        // H psi_0 = mc2 a0 + c (p0 - i p1) a1 ; H psi_1 = c (p0 + i p1) a0 - mc2 a1
-                        const C h0 = mk<C>(fm * a0.x + f0 * a1.x + f1 * a1.y, fm * a0.y + f0 * a1.y - f1 * a1.x);
-                        const C h1 = mk<C>(f0 * a0.x - f1 * a0.y - fm * a1.x, f0 * a0.y + f1 * a0.x - fm * a1.y);
-                        y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
-                        y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
-                    } else {
-                        const C a0 = y[0][i], a1 = y[1][i], a2 = y[2][i], a3 = y[3][i];
-                        // sigma.p (v0, v1) = (p2 v0 + (p0 - i p1) v1, (p0 + i p1) v0 - p2 v1)
-                        // H psi = (mc2 u + c sigma.p l, c sigma.p u - mc2 l)
-                        const C h0 = mk<C>(fm * a0.x + f2 * a2.x + f0 * a3.x + f1 * a3.y, fm * a0.y + f2 * a2.y + f0 * a3.y - f1 * a3.x);
-                        const C h1 = mk<C>(fm * a1.x + f0 * a2.x - f1 * a2.y - f2 * a3.x, fm * a1.y + f0 * a2.y + f1 * a2.x - f2 * a3.y);
-                        const C h2 = mk<C>(f2 * a0.x + f0 * a1.x + f1 * a1.y - fm * a2.x, f2 * a0.y + f0 * a1.y - f1 * a1.x - fm * a2.y);
-                        const C h3 = mk<C>(f0 * a0.x - f1 * a0.y - f2 * a1.x - fm * a3.x, f0 * a0.y + f1 * a0.x - f2 * a1.y - fm * a3.y);
-                        y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
-                        y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
-                        y[2][i] = mk<C>(fc * a2.x + h2.y, fc * a2.y - h2.x);
-                        y[3][i] = mk<C>(fc * a3.x + h3.y, fc * a3.y - h3.x);
-                    }
-                }
-#pragma unroll
-                for (int c2 = 0; c2 < CC; ++c2)
-#pragma unroll
-                    for (int i = 0; i < PP; ++i) sm[(c2 * TL + t) * a.pitch + padp(u * 16 + c * PP + i)] = y[c2][i];
-                __syncthreads();
-#pragma unroll
-                for (int q = 0; q < 16; ++q) x[q] = sl[padp(u * 16 + q)];
             }
         }
 
-        if (a.do_dit) DitChain<T, N, LAST, -SIGN>::run(x, u, tw, sl);
+        for (int rep = 0; rep < a.nrep; ++rep) {
+            const long long n = a.n0 + rep;
+            if (a.pre_v && rep == 0) natural_v(a.pre_v, n, n, false);
 
-        if (a.post_v) {
-            if (rep + 1 < a.nrep) natural_v(a.post_v, n, n + 1, true);
-            else natural_v(a.post_v, n, n, false);
+            if (a.do_dif) DifChain<T, N, 0, SIGN>::run(x, u, stw, sl);
+
+            if (a.mid_on) {
+                if constexpr (PW == PW_V) {
+                    // merged or half potential phase in the permuted order: register q of thread u is
+                    // table slot q U + u (coalesced across u)
+                    if (a.field_kind == 1 && u == 0) lsc[t] = expi<T>(-other_axes_angle(n, n + 1, a.v_mid_full != 0));
+                    if (a.field_kind == 1) __syncthreads();
+                    const long long vb = line * (long long)N + u;
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) {
+                        C h;
+                        if (a.vrep == VREP_TABLE) {
+                            h = reinterpret_cast<const C *>(a.vtab)[vb + q * U];
+                            if (a.v_mid_full) h = cmul(h, h);
+                        } else {
+                            const double ang = reinterpret_cast<const double *>(a.vtab)[vb + q * U];
+                            h = expi<T>(a.v_mid_full ? 2.0 * ang : ang);
+                        }
+                        if (a.field_kind == 1) h = cmul(h, lsc[t]);
+                        if (a.ephase) h = cmul(h, reinterpret_cast<const C *>(a.ephase)[q * U + u]);
+                        x[q] = cmul(x[q], h);
+                    }
+                } else if constexpr (PW == PW_KS) {
+                    const bool has_lsc = a.kph1 || a.kph2;
+                    const C *__restrict__ k0 = reinterpret_cast<const C *>(a.kph0);
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) {
+                        C f = k0[q * U + u];
+                        if (has_lsc) f = cmul(f, lsc[t]);
+                        x[q] = cmul(x[q], f);
+                    }
+                } else if constexpr (PW == PW_KD2 || PW == PW_KD4) {
+                    constexpr int PP = 16 / CC;
+                    // shift of the kinetic momentum: pi = k - q Abar_n (reading G16)
+                    double sh[3] = {0.0, 0.0, 0.0};
+                    if (a.field_kind == 2)
+                        for (int ax = 0; ax < a.ndim; ++ax) sh[ax] = a.charge * favg(a, n, ax);
+                    // non-line momenta of this line: the line axis is axis 0 here
+                    double p1 = 0.0, p2 = 0.0;
+                    if (a.ndim == 2) p1 = a.kv2[ib] - sh[1];
+                    if (a.ndim == 3) {
+                        p1 = a.kv1[ia] - sh[1];
+                        p2 = a.kv2[ib] - sh[2];
+                    }
+                    // all components of a k point into one thread: thread (c, u) takes the PP points
+                    // 16 u + c PP + i of every component
+                    C *me = sl + 17 * u;
+                    __syncthreads();
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) me[q] = x[q];
+                    __syncthreads();
+                    C y[CC][PP];
+#pragma unroll
+                    for (int c2 = 0; c2 < CC; ++c2)
+#pragma unroll
+                        for (int i = 0; i < PP; ++i) y[c2][i] = sm[(c2 * TL + t) * a.pitch + 17 * u + c * PP + i];
+                    const double mc2 = a.mass * a.clight * a.clight;
+#pragma unroll
+                    for (int i = 0; i < PP; ++i) {
+                        const int q2 = c * PP + i;
+                        const double p0 = a.kv0[q2 * U + u] - sh[0];
+                        const double pp = p0 * p0 + p1 * p1 + p2 * p2;
+                        const double E = sqrt(a.clight * a.clight * pp + mc2 * mc2);
+                        double sn, cs;
+                        sincos(E * a.dt, &sn, &cs);
+                        double sE = E > 0.0 ? sn / E : a.dt;
+                        cs *= a.scale;
+                        sE *= a.scale;
+                        const T fc = (T)cs;
+                        const T fm = (T)(sE * mc2);
+                        const T f0 = (T)(sE * a.clight * p0), f1 = (T)(sE * a.clight * p1), f2 = (T)(sE * a.clight * p2);
+                        // out = cs psi - i sE H psi ;  (-i)(a + i b) = b - i a
+                        if constexpr (CC == 2) {
+                            const C a0 = y[0][i], a1 = y[1][i];
+                            // H psi_0 = mc2 a0 + c (p0 - i p1) a1 ; H psi_1 = c (p0 + i p1) a0 - mc2 a1
+                            const C h0 = mk<C>(fm * a0.x + f0 * a1.x + f1 * a1.y, fm * a0.y + f0 * a1.y - f1 * a1.x);
+                            const C h1 = mk<C>(f0 * a0.x - f1 * a0.y - fm * a1.x, f0 * a0.y + f1 * a0.x - fm * a1.y);
+                            y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
+                            y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
+                        } else {
+                            const C a0 = y[0][i], a1 = y[1][i], a2 = y[2][i], a3 = y[3][i];
+                            // sigma.p (v0, v1) = (p2 v0 + (p0 - i p1) v1, (p0 + i p1) v0 - p2 v1)
+                            // H psi = (mc2 u + c sigma.p l, c sigma.p u - mc2 l)
+                            const C h0 = mk<C>(fm * a0.x + f2 * a2.x + f0 * a3.x + f1 * a3.y, fm * a0.y + f2 * a2.y + f0 * a3.y - f1 * a3.x);
+                            const C h1 = mk<C>(fm * a1.x + f0 * a2.x - f1 * a2.y - f2 * a3.x, fm * a1.y + f0 * a2.y + f1 * a2.x - f2 * a3.y);
+                            const C h2 = mk<C>(f2 * a0.x + f0 * a1.x + f1 * a1.y - fm * a2.x, f2 * a0.y + f0 * a1.y - f1 * a1.x - fm * a2.y);
+                            const C h3 = mk<C>(f0 * a0.x - f1 * a0.y - f2 * a1.x - fm * a3.x, f0 * a0.y + f1 * a0.x - f2 * a1.y - fm * a3.y);
+                            y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
+                            y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
+                            y[2][i] = mk<C>(fc * a2.x + h2.y, fc * a2.y - h2.x);
+                            y[3][i] = mk<C>(fc * a3.x + h3.y, fc * a3.y - h3.x);
+                        }
+                    }
+#pragma unroll
+                    for (int c2 = 0; c2 < CC; ++c2)
+#pragma unroll
+                        for (int i = 0; i < PP; ++i) sm[(c2 * TL + t) * a.pitch + 17 * u + c * PP + i] = y[c2][i];
+                    __syncthreads();
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) x[q] = me[q];
+                }
+            }
+
+            if (a.do_dit) DitChain<T, N, LAST, -SIGN>::run(x, u, stw, sl);
+
+            if (a.post_v) {
+                if (rep + 1 < a.nrep) natural_v(a.post_v, n, n + 1, true);
+                else natural_v(a.post_v, n, n, false);
+            }
         }
+
+        if (!a.do_dit && a.unpermute) {
+            // registers hold frequency revB[u] + U q at position 16 u + q: scatter to natural order
+            C *wa = sl + padp(a.revB[u]);
+            const C *rb = sl + padp(u);
+            __syncthreads();
+#pragma unroll
+            for (int q = 0; q < 16; ++q) wa[lin_delta(q, U)] = x[q];
+            __syncthreads();
+#pragma unroll
+            for (int q = 0; q < 16; ++q) x[q] = rb[lin_delta(q, U)];
+        }
+        if (a.do_dit || a.unpermute || a.dbg_copy) {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) st_stream(&gp[(long long)(u + q * U) * estep], x[q]);
+        } else {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) st_stream(&gp[(long long)(u * 16 + q) * estep], x[q]);
+        }
+
+        wtile = ntile;
+        parity ^= 1;
+        __syncthreads();  // everyone is done with the exchange buffer, lsc and the mailbox slot
     }
 
-    if (!a.do_dit && a.unpermute) {
-        // registers hold frequency revB[u] + U q at position 16 u + q: scatter to natural order
-        const int rb = a.revB[u];
-        __syncthreads();
-#pragma unroll
-        for (int q = 0; q < 16; ++q) sl[padp(rb + q * U)] = x[q];
-        __syncthreads();
-#pragma unroll
-        for (int q = 0; q < 16; ++q) x[q] = sl[padp(u + q * U)];
-    }
-    if (a.do_dit || a.unpermute) {
-#pragma unroll
-        for (int q = 0; q < 16; ++q) gp[(long long)(u + q * U) * estep] = x[q];
-    } else {
-#pragma unroll
-        for (int q = 0; q < 16; ++q) gp[(long long)(u * 16 + q) * estep] = x[q];
+    // the last CTA to leave resets the scheduler for the next launch on this stream
+    if (tid == 0) {
+        __threadfence();
+        const unsigned done = atomicAdd(&a.sched[1], 1u);
+        if (done == gridDim.x - 1) {
+            a.sched[0] = 0u;
+            a.sched[1] = 0u;
+            __threadfence();
+        }
     }
 }
 
-// host-side launcher, explicitly instantiated per (T, N) in sso_inst_*.cu
+// host-side launcher, explicitly instantiated per (T, N) in sso_inst.cu
 template <typename T, int N, bool STRIDED, int PW, int SIGN>
-cudaError_t launch_pass(const PassArgs &a, unsigned grid, unsigned threads, size_t smem, cudaStream_t st);
+cudaError_t launch_pass(const PassArgs &a, unsigned threads, size_t smem, cudaStream_t st);
 
 }  // namespace sso
