@@ -1,0 +1,306 @@
+#!/usr/bin/env python
+"""bench.py -- grid-point updates/s of the Fourier split-operator step on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 2a] [--impl reference]
+
+One bench "step" is one pass of the whole hot path over one batch: a single call of
+sso_step(psi, SPLIT_STEPS) that advances the wavefunction by SPLIT_STEPS = 128 split-operator time steps
+(the paper's protocol: 128 time steps, one upload before and one download after).
+  value  device-resident throughput: psi, the potential table and the field table are in HBM before the
+         timed region; K calls timed with CUDA events on the launching stream.
+  e2e    the same K calls through sso_step_host on a pinned HOST buffer: every call uploads psi, steps and
+         downloads it inside the timed region.
+  roofline  HBM: algorithmic bytes of one pass-kernel launch (one read + one write of psi, DESIGN.md
+         "Bytes") / average pass-kernel launch duration over the timed region, against MEASURED_PEAKS.json.
+  cpu_baseline  the oracle as it stands on the host cores, bounded sample, rank 0 at N=1 only.
+Workload at N=1: BASELINE.json configs[1], complex128 ("2a": 2D Schroedinger 2048^2 with a dipole field).
+N>1: replicas only: every rank runs the same workload on its own GPU, no
+data-path collective; value = all ranks' updates / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+import workloads as wl  # noqa: E402
+
+METRIC = "grid-point updates/s per split-operator step"
+UNIT = "grid-point updates/s"
+SPLIT_STEPS = 128  # split-operator steps per sso_step call ("over 128 time steps")
+
+# name -> (config number, precision name, passes P per steady-state step)
+WORKLOADS = {
+    "1": (1, "c128", 1), "2a": (2, "c128", 2), "2b": (2, "c64", 2), "3": (3, "c128", 4), "4": (4, "c128", 2), "5": (5, "c128", 4),
+}
+DESCR = {
+    "1": "cfg1 1D Schroedinger 4096, harmonic well, complex128",
+    "2a": "cfg2 2D Schroedinger 2048x2048, soft-core Coulomb + dipole field E(t), complex128",
+    "2b": "cfg2 2D Schroedinger 2048x2048, soft-core Coulomb + dipole field E(t), complex64",
+    "3": "cfg3 3D Schroedinger 256^3, 32 random Gaussians, complex128",
+    "4": "cfg4 2D Dirac 2 components 1024x1024, soft-core Coulomb + A(t) in the kinetic unitary, complex128",
+    "5": "cfg5 3D Dirac 4 components 256^3, soft-core Coulomb, complex128",
+}
+# dram__bytes_read.sum + dram__bytes_write.sum per pass-kernel launch from the committed `ncu --set full`
+# capture (profiles/, see the .md beside each); None where no capture exists yet
+NCU_TRAFFIC_BYTES = {}
+
+
+def load_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, device copy)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def make_workload(name: str, nrows: int):
+    cfg, prec, P = WORKLOADS[name]
+    w = wl.CONFIGS[cfg](nsteps=nrows)
+    return w, prec, P
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)
+        self.proc.terminate()
+        inside = [r for t, r in self.rows if t0 <= t <= t1] or [r for _, r in self.rows[-3:]]
+        mhz, mx, reasons = [], None, set()
+        for r in inside:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                mhz.append(float(f[0]))
+                mx = float(f[1])
+            except ValueError:
+                continue
+            for nm, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(mhz)) if mhz else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(mhz)}
+
+
+def oracle_rate(w, seconds_target: float = 12.0):
+    """The oracle as it stands, all host cores it uses, on a bounded sample of split steps of the same workload."""
+    import oracle
+
+    o = oracle.Solver(w.sizes, w.dx, w.dt, w.ncomp, w.mass, w.c, w.charge)
+    o.set_potential(w.V)
+    if w.field_kind:
+        o.set_field(w.field_kind, w.step_avg)
+    psi = w.psi0
+    t0 = time.perf_counter()
+    psi = o.step(psi, 1)
+    one = time.perf_counter() - t0
+    n = int(max(1, min(w.step_avg.shape[0] - 1 if w.field_kind else 10**9, seconds_target / max(one, 1e-6))))
+    t0 = time.perf_counter()
+    o.step(psi, n)
+    dt = time.perf_counter() - t0
+    return w.npoints * n / dt, n, oracle.max_threads(), dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same config/metric/unit; each bench step is a bounded
+    sample of the workload (REF_SPLIT split-operator steps instead of 128)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+
+    name = args.workload
+    REF_SPLIT = {"1": 128, "2a": 4, "2b": 4, "3": 1, "4": 8, "5": 1}[name]
+    w, prec, P = make_workload(name, REF_SPLIT * (args.steps + args.warmup) + 1)
+    o = oracle.Solver(w.sizes, w.dx, w.dt, w.ncomp, w.mass, w.c, w.charge)
+    o.set_potential(w.V)
+    if w.field_kind:
+        o.set_field(w.field_kind, w.step_avg)
+    psi = w.psi0 if prec == "c128" else w.psi0.astype(np.complex64).astype(np.complex128)
+    for _ in range(args.warmup):
+        psi = o.step(psi, REF_SPLIT)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        psi = o.step(psi, REF_SPLIT)
+    dt = time.perf_counter() - t0
+    value = w.npoints * REF_SPLIT * args.steps / dt
+    sample = f"{REF_SPLIT} split-operator steps per bench step (of {SPLIT_STEPS}), full grid, fp64"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": DESCR[name], "split_steps_per_step": REF_SPLIT, "grid": list(w.sizes), "ncomp": w.ncomp},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_product(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1012_3911_b200 as sso
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    name = args.workload
+    K, W = args.steps, args.warmup
+    nrows = SPLIT_STEPS  # every call replays field rows 0..127 (sso_set_time_index(0) before each call)
+    w, prec, P = make_workload(name, nrows)
+    precision = sso.C128 if prec == "c128" else sso.C64
+    cdt = np.complex128 if prec == "c128" else np.complex64
+    esz = 16 if prec == "c128" else 8
+    S = w.npoints * w.ncomp * esz
+
+    plan = sso.Plan(w.sizes, w.dx, w.dt, w.ncomp, precision)
+    plan.set_constants(w.mass, w.c, w.charge)
+    plan.set_potential(w.V)
+    if w.field_kind:
+        plan.set_field(w.field_kind, np.ascontiguousarray(w.step_avg))
+    psi0 = w.psi0.astype(cdt)
+    psi = torch.from_numpy(psi0).cuda()
+    stream = torch.cuda.current_stream()
+
+    def call():
+        plan.set_time_index(0)
+        plan.step(psi, SPLIT_STEPS, stream=stream)
+
+    for _ in range(max(W, 3) if W else 0):
+        call()
+    launches_per_call = plan.launch_count(SPLIT_STEPS)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.15)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.time()
+    e0.record(stream)
+    for _ in range(K):
+        call()
+    e1.record(stream)
+    barrier()
+    t1 = time.time()
+    ms = e0.elapsed_time(e1)
+    norm_after = plan.norm(psi)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
+
+    # end to end: host buffer in, host buffer out, copies inside the timed region
+    host = torch.from_numpy(psi0.copy()).pin_memory()
+    for _ in range(2):
+        plan.set_time_index(0)
+        plan.step_host(host, SPLIT_STEPS)
+    host.copy_(torch.from_numpy(psi0))
+    barrier()
+    h0 = time.perf_counter()
+    for _ in range(K):
+        plan.set_time_index(0)
+        plan.step_host(host, SPLIT_STEPS)  # synchronous: returns after the download
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - h0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_norm = float(np.sum(np.abs(host.numpy().astype(np.complex128)) ** 2) * np.prod(w.dx))
+
+    updates = float(w.npoints) * SPLIT_STEPS * K * world
+    value = updates / (ms * 1e-3)
+    if rank == 0:
+        peak, peak_src = load_peaks()
+        pass_launches = K * (SPLIT_STEPS * P + (1 if len(w.sizes) > 1 else 0)) if len(w.sizes) > 1 else K
+        per_launch_s = ms * 1e-3 / pass_launches
+        bytes_per_launch = 2.0 * S if len(w.sizes) > 1 else 2.0 * S  # one read + one write of psi
+        achieved = bytes_per_launch / per_launch_s / 1e9
+        traffic = NCU_TRAFFIC_BYTES.get(name)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if prec == "c128" else "f32", "data": "synthetic",
+            "config": {"workload": DESCR[name], "split_steps_per_step": SPLIT_STEPS, "grid": list(w.sizes), "ncomp": w.ncomp,
+                       "parallelism": "replicas" if world > 1 else "single GPU", "us_per_split_step": ms * 1e3 / (K * SPLIT_STEPS),
+                       "l2": "no flush: psi + potential phase table streamed per split step = %.0f MB (L2 is 126 MB)" % (2 * S / 1e6 if name != "2b" else 2 * S / 1e6),
+                       "norm_after": norm_after},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                         "kernel": "sso::pass_kernel", "bytes_per_launch": bytes_per_launch, "avg_launch_us": per_launch_s * 1e6,
+                         "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
+            "e2e": {"value": updates / e2e_s, "unit": UNIT, "h2d_bytes_per_step": S, "d2h_bytes_per_step": S, "norm_after": e2e_norm},
+            "gpu_launches": int(launches_per_call * K),
+            "clocks": clocks,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            v, n, cores, secs = oracle_rate(w)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{n} split-operator steps of the same full-size workload in {secs:.1f} s (fp64)"}
+        print(json.dumps(line), flush=True)
+    plan.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="sso", choices=["sso", "reference"])
+    ap.add_argument("--workload", default="2a", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_product(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,211 @@
+"""BASELINE.json's configs at their FULL sizes, in the launch configuration bench.py times (default options):
+a few oracle steps element by element where the oracle finishes in seconds, one-by-one sampled outputs
+through the O(N) definition sum, and the size-independent properties (unitarity, reversibility).  Plus the
+boundary's edge cases on the GPU.
+"""
+import ctypes
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_1012_3911_b200 as sso
+import workloads as wl
+from test_parity_gpu import TOL, gpu_steps, make_oracle, make_plan, oracle_steps, rel_l2, start_state, torch  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+FULL = [
+    ("cfg2a", lambda: wl.config2(nsteps=8), sso.C128, 3),
+    ("cfg2b", lambda: wl.config2(nsteps=8), sso.C64, 3),
+    ("cfg4", lambda: wl.config4(nsteps=8), sso.C128, 3),
+    ("cfg3", lambda: wl.config3(nsteps=4), sso.C128, 2),
+    ("cfg5", lambda: wl.config5(nsteps=2), sso.C128, 1),
+]
+
+
+@pytest.mark.parametrize("name,make,prec,nsteps", FULL, ids=[f[0] for f in FULL])
+def test_full_size_first_steps_and_samples(torch, name, make, prec, nsteps):
+    w = make()
+    got, nrm = gpu_steps(torch, w, nsteps, prec)
+    want = oracle_steps(w, nsteps, prec)
+    err = rel_l2(got.astype(np.complex128), want)
+    assert err <= TOL[prec] * 0.1, (name, err)
+    assert abs(nrm - 1.0) < (1e-12 if prec == sso.C128 else 1e-5)
+    # sampled outputs of step `nsteps`, each computed on its own from the definition (O(N) sum per sample):
+    # oracle state after nsteps-1 steps -> V/2, forward DFT -> K -> one inverse-DFT sum + V/2 per sample
+    o = make_oracle(w)
+    prev = o.step(start_state(w, prec).astype(np.complex128), nsteps - 1) if nsteps > 1 else start_state(w, prec).astype(np.complex128)
+    psik = o.half_step_to_k(prev, nsteps - 1)
+    rng = np.random.default_rng(99)
+    centre = int(np.ravel_multi_index([n // 2 for n in w.sizes], w.sizes))
+    idx = [centre, 0, w.npoints - 1] + [int(i) for i in rng.integers(0, w.npoints, size=5)]
+    flat = got.reshape(w.ncomp, -1)
+    scale = np.abs(want).max()
+    for i in idx:
+        s = o.inverse_sample(psik, nsteps - 1, i)
+        assert np.abs(flat[:, i] - s).max() <= TOL[prec] * scale, (name, i)
+
+
+@pytest.mark.parametrize("cfg,prec", [(2, sso.C128), (2, sso.C64), (3, sso.C128), (4, sso.C128), (5, sso.C128)])
+def test_full_size_unitarity_and_reversibility(torch, cfg, prec):
+    """Strang step is unitary and symmetric: the norm stays 1 and stepping with -dt (fields replayed
+    backwards) returns psi0 (eq. 7).  Holds at any size; run at BASELINE's sizes."""
+    nsteps = {2: 20, 3: 6, 4: 20, 5: 4}[cfg]
+    w = wl.CONFIGS[cfg](nsteps=nsteps)
+    p = make_plan(w, prec)
+    s0 = start_state(w, prec)
+    psi = torch.from_numpy(s0).cuda()
+    p.step(psi, nsteps)
+    n1 = p.norm(psi)
+    assert abs(n1 - 1.0) < (1e-12 if prec == sso.C128 else 2e-5), n1
+    moved = rel_l2(psi.cpu().numpy(), s0)
+    assert moved > 1e-4  # the step did something
+    back = sso.Plan(w.sizes, w.dx, -w.dt, w.ncomp, prec)
+    back.set_constants(w.mass, w.c, w.charge)
+    back.set_potential(w.V)
+    if w.field_kind:
+        back.set_field(w.field_kind, np.ascontiguousarray(w.step_avg[:nsteps][::-1]))
+    back.step(psi, nsteps)
+    torch.cuda.synchronize()
+    err = rel_l2(psi.cpu().numpy(), s0)
+    assert err <= (1e-12 if prec == sso.C128 else 2e-5), err
+    p.destroy()
+    back.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# edge cases of the boundary
+# ---------------------------------------------------------------------------------------------------------
+
+def test_zero_steps_and_chunking(torch):
+    w = wl.config2(sizes=(64, 128), nsteps=12)
+    p = make_plan(w)
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    p.step(psi, 0)
+    torch.cuda.synchronize()
+    assert np.array_equal(psi.cpu().numpy(), w.psi0)
+    assert p.get_time_index() == 0 and p.launch_count(0) == 0
+    one, _ = gpu_steps(torch, w, 12)
+    many, _ = gpu_steps(torch, w, 12, chunks=[1] * 12)
+    assert rel_l2(many, one) < 1e-14
+    want = oracle_steps(w, 12)
+    assert rel_l2(one, want) < 1e-13 and rel_l2(many, want) < 1e-13
+    p.destroy()
+
+
+def test_time_index_selects_the_field_row(torch):
+    w = wl.config4(sizes=(64, 64), nsteps=10)
+    p = make_plan(w)
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    p.set_time_index(5)
+    p.step(psi, 3)
+    torch.cuda.synchronize()
+    o = make_oracle(w)
+    o.set_time_index(5)
+    assert rel_l2(psi.cpu().numpy(), o.step(w.psi0, 3)) < 1e-13
+    assert p.get_time_index() == 8
+    p.destroy()
+
+
+def test_error_paths_on_device(torch):
+    w = wl.config2(sizes=(32, 32), nsteps=4)
+    p = make_plan(w)
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    before = psi.clone()
+    with pytest.raises(sso.SsoError) as e:
+        p.step(psi, w.step_avg.shape[0] + 1)  # field table too short
+    assert e.value.code == sso.ERR_STATE
+    with pytest.raises(sso.SsoError) as e:
+        p.step(psi.data_ptr() + 8, 1)  # misaligned
+    assert e.value.code == sso.ERR_INVALID
+    with pytest.raises(sso.SsoError) as e:
+        p.step(psi, -1)
+    assert e.value.code == sso.ERR_INVALID
+    with pytest.raises(sso.SsoError):
+        p.step(None, 1)
+    with pytest.raises(sso.SsoError):
+        p.set_field(7, w.step_avg)
+    with pytest.raises(sso.SsoError):
+        p.set_field(sso.FIELD_E, np.full((2, 2), np.nan))
+    with pytest.raises(sso.SsoError):
+        p.set_constants(-1.0, 1.0, 1.0)
+    with pytest.raises(sso.SsoError):
+        p.set_option(sso.OPT_LINES_PER_TILE_CONTIG, 3)
+    with pytest.raises(sso.SsoError):
+        p.set_time_index(-1)
+    torch.cuda.synchronize()
+    assert torch.equal(psi, before)  # failed calls touched nothing
+    p.destroy()
+    p.destroy()  # idempotent
+
+
+def test_potential_sources_agree(torch):
+    """Host V, device V and V = NULL (zero) through sso_set_potential."""
+    w = wl.config3(sizes=(16, 32, 32), nsteps=3)
+    a, _ = gpu_steps(torch, w, 3)
+    p = make_plan(w)
+    p.set_potential(torch.from_numpy(w.V).cuda(), on_device=True)
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    p.step(psi, 3)
+    torch.cuda.synchronize()
+    assert np.array_equal(psi.cpu().numpy(), a)
+    p.set_potential(None)
+    p.set_time_index(0)
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    p.step(psi, 3)
+    torch.cuda.synchronize()
+    w0 = wl.Workload("free", w.sizes, w.dx, w.dt, 1, 3, w.psi0, V=None)
+    assert rel_l2(psi.cpu().numpy(), oracle_steps(w0, 3)) < 1e-13
+    p.destroy()
+
+
+def test_tile_options_and_angle_table_do_not_change_results(torch):
+    w = wl.config2(sizes=(128, 256), nsteps=6)
+    want = oracle_steps(w, 6)
+    for opts in (((sso.OPT_LINES_PER_TILE_CONTIG, 1), (sso.OPT_LINES_PER_TILE_STRIDED, 1)),
+                 ((sso.OPT_LINES_PER_TILE_CONTIG, 4), (sso.OPT_LINES_PER_TILE_STRIDED, 8)),
+                 ((sso.OPT_POTENTIAL_PHASE, 1),)):
+        got, _ = gpu_steps(torch, w, 6, options=opts)
+        assert rel_l2(got, want) < 1e-13, opts
+
+
+def test_step_host_matches_device_path(torch):
+    w = wl.config4(sizes=(64, 128), nsteps=5)
+    dev, _ = gpu_steps(torch, w, 5)
+    p = make_plan(w)
+    host = torch.from_numpy(w.psi0.copy()).pin_memory()
+    p.step_host(host, 5)
+    assert np.array_equal(host.numpy(), dev)
+    p.destroy()
+
+
+def test_norm_matches_oracle(torch):
+    for prec in (sso.C128, sso.C64):
+        w = wl.config5(sizes=(16, 16, 32), nsteps=1)
+        s = start_state(w, prec)
+        p = make_plan(w, prec)
+        got = p.norm(torch.from_numpy(s).cuda())
+        want = make_oracle(w).norm(s.astype(np.complex128))
+        assert abs(got - want) <= 1e-14 * want
+        p.destroy()
+
+
+def test_steps_on_a_side_stream_and_graph_capture(torch):
+    """sso_step only enqueues kernels on the caller's stream, so it can be captured into a CUDA graph."""
+    w = wl.config2(sizes=(64, 64), nsteps=8)
+    p = make_plan(w)
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(st):
+        p.step(psi, 2, stream=st)  # warm-up builds the static tables outside the capture
+    st.synchronize()
+    g = torch.cuda.CUDAGraph()
+    p.set_time_index(2)
+    with torch.cuda.graph(g, stream=st):
+        p.step(psi, 3, stream=torch.cuda.current_stream())
+    g.replay()
+    torch.cuda.synchronize()
+    assert rel_l2(psi.cpu().numpy(), oracle_steps(w, 5)) < 1e-13
+    p.destroy()

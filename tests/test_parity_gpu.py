@@ -1,0 +1,177 @@
+"""GPU parity: the CUDA path (through the C ABI of include/sso.h) against the CPU oracle, element by element,
+on the same seeded inputs (workloads.py).  Metric and bars (BASELINE.json north_star, G19):
+relative L2 error over all components  <= 1e-11 (complex128) / <= 2e-5 (complex64)  after 100 steps.
+For complex64 the oracle starts from the complex64-rounded psi0 promoted to double.
+"""
+import ctypes
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_1012_3911_b200 as sso
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = {sso.C128: 1e-11, sso.C64: 2e-5}
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+
+    assert t.cuda.is_available()
+    t.cuda.set_device(0)
+    sso.lib()  # fails loudly if libsso.so is missing: there is no fallback
+    return t
+
+
+def rel_l2(got, want):
+    return float(np.linalg.norm((got - want).ravel()) / np.linalg.norm(want.ravel()))
+
+
+def make_plan(w, prec=sso.C128):
+    p = sso.Plan(w.sizes, w.dx, w.dt, w.ncomp, prec)
+    p.set_constants(w.mass, w.c, w.charge)
+    p.set_potential(w.V)
+    if w.field_kind:
+        p.set_field(w.field_kind, np.ascontiguousarray(w.step_avg))
+    return p
+
+
+def make_oracle(w):
+    o = oracle.Solver(w.sizes, w.dx, w.dt, w.ncomp, w.mass, w.c, w.charge)
+    o.set_potential(w.V)
+    if w.field_kind:
+        o.set_field(w.field_kind, w.step_avg)
+    return o
+
+
+def start_state(w, prec):
+    return w.psi0.astype(np.complex128 if prec == sso.C128 else np.complex64)
+
+
+def gpu_steps(torch, w, nsteps, prec=sso.C128, chunks=None, psi0=None, options=()):
+    p = make_plan(w, prec)
+    for o, v in options:
+        p.set_option(o, v)
+    if options:
+        p.set_potential(w.V)
+    psi = torch.from_numpy(start_state(w, prec) if psi0 is None else psi0).cuda()
+    for c in chunks or [nsteps]:
+        p.step(psi, c)
+    torch.cuda.synchronize()
+    nrm = p.norm(psi)
+    p.destroy()
+    return psi.cpu().numpy(), nrm
+
+
+def oracle_steps(w, nsteps, prec=sso.C128, psi0=None):
+    o = make_oracle(w)
+    s = (start_state(w, prec) if psi0 is None else psi0).astype(np.complex128)
+    return o.step(s, nsteps)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# 100-step parity on reduced grids of every config: several tiles per pass, non-square shapes
+# ---------------------------------------------------------------------------------------------------------
+REDUCED = [
+    ("cfg1", lambda: wl.config1(sizes=(1024,), nsteps=100), sso.C128),
+    ("cfg2a", lambda: wl.config2(sizes=(256, 512), nsteps=100), sso.C128),
+    ("cfg2b", lambda: wl.config2(sizes=(256, 512), nsteps=100), sso.C64),
+    ("cfg2a_tall", lambda: wl.config2(sizes=(1024, 64), nsteps=100), sso.C128),
+    ("cfg3", lambda: wl.config3(sizes=(32, 64, 128), nsteps=100), sso.C128),
+    ("cfg4", lambda: wl.config4(sizes=(256, 128), nsteps=100), sso.C128),
+    ("cfg5", lambda: wl.config5(sizes=(32, 16, 64), nsteps=100), sso.C128),
+    ("dirac1d_c2", lambda: wl.dirac1d(sizes=(512,), nsteps=100, ncomp=2), sso.C128),
+    ("dirac1d_c4", lambda: wl.dirac1d(sizes=(512,), nsteps=100, ncomp=4), sso.C128),
+    ("cfg4_c64", lambda: wl.config4(sizes=(128, 128), nsteps=100), sso.C64),
+    ("cfg3_c64", lambda: wl.config3(sizes=(32, 32, 64), nsteps=100), sso.C64),
+]
+
+
+@pytest.mark.parametrize("name,make,prec", REDUCED, ids=[r[0] for r in REDUCED])
+def test_parity_100_steps_reduced(torch, name, make, prec):
+    w = make()
+    got, nrm = gpu_steps(torch, w, 100, prec)
+    want = oracle_steps(w, 100, prec)
+    err = rel_l2(got.astype(np.complex128), want)
+    assert err <= TOL[prec], (name, err)
+    # element by element as well: no single point may be off by more than the bar times the peak amplitude
+    peak = np.abs(want).max()
+    assert np.abs(got - want).max() <= 50 * TOL[prec] * peak
+    assert abs(nrm - 1.0) < (1e-11 if prec == sso.C128 else 1e-4)
+
+
+def test_config1_full_size_100_and_1000_steps(torch):
+    """BASELINE config 1 at its full size, parity recorded at 100 and 1000 steps."""
+    w = wl.config1()
+    o = make_oracle(w)
+    p = make_plan(w)
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    ref = w.psi0
+    for upto, n in ((100, 100), (1000, 900)):
+        p.step(psi, n)
+        ref = o.step(ref, n)
+        torch.cuda.synchronize()
+        err = rel_l2(psi.cpu().numpy(), ref)
+        assert err <= 1e-11, (upto, err)
+    assert p.get_time_index() == 1000
+    p.destroy()
+
+
+def test_random_state_all_axis_lengths(torch):
+    """Every supported line length, noise input (all k populated), contiguous and strided passes."""
+    for n in (16, 32, 64, 128, 256, 512, 1024, 2048, 4096):
+        for sizes in ((n,), (n, 16), (16, n)):
+            dx = (0.1,) * len(sizes)
+            psi0 = wl.random_state(sizes, 1, seed=n + len(sizes), dx=dx)
+            rng = np.random.default_rng(n)
+            V = rng.uniform(-1, 1, size=sizes)
+            w = wl.Workload("rand", sizes, dx, 0.01, 1, 3, psi0, V=V)
+            got, _ = gpu_steps(torch, w, 3)
+            want = oracle_steps(w, 3)
+            assert rel_l2(got, want) <= 1e-13, (sizes, rel_l2(got, want))
+
+
+def test_random_state_3d_and_dirac(torch):
+    for ncomp, sizes in ((1, (16, 32, 64)), (4, (64, 16, 32)), (2, (128, 64)), (4, (64, 128)), (4, (2048,)), (2, (4096,))):
+        dx = (0.05,) * len(sizes)
+        psi0 = wl.random_state(sizes, ncomp, seed=7 * ncomp + len(sizes), dx=dx)
+        rng = np.random.default_rng(ncomp)
+        V = rng.uniform(-50, 50, size=sizes)
+        nd = len(sizes)
+        avg = rng.uniform(-3, 3, size=(8, nd))
+        w = wl.Workload("rand", sizes, dx, 2e-4, ncomp, 4, psi0, V=V, field_kind=wl.FIELD_A, step_avg=avg)
+        got, _ = gpu_steps(torch, w, 4)
+        want = oracle_steps(w, 4)
+        assert rel_l2(got, want) <= 1e-13, (ncomp, sizes, rel_l2(got, want))
+
+
+def test_field_e_on_every_axis(torch):
+    """Length-gauge field with components along all axes (the last axis uses the per-step line phase table)."""
+    for sizes in ((64,), (32, 64), (16, 32, 64)):
+        nd = len(sizes)
+        dx = (0.2,) * nd
+        rng = np.random.default_rng(nd)
+        psi0 = wl.random_state(sizes, 1, seed=nd, dx=dx)
+        w = wl.Workload("e", sizes, dx, 0.01, 1, 5, psi0, V=rng.uniform(-1, 1, size=sizes), field_kind=wl.FIELD_E,
+                        step_avg=rng.uniform(-0.5, 0.5, size=(6, nd)))
+        got, _ = gpu_steps(torch, w, 5)
+        assert rel_l2(got, oracle_steps(w, 5)) <= 1e-13
+        got2, _ = gpu_steps(torch, w, 5, chunks=[2, 1, 2])
+        assert rel_l2(got2, got) <= 1e-14  # merged potential phases equal unmerged ones up to rounding
+
+
+def test_schroedinger_with_vector_potential(torch):
+    """SSO_FIELD_A for ncomp = 1: kinetic tables rebuilt per step (eq. 13 with the shift, reading G17)."""
+    for sizes in ((128,), (32, 64)):
+        nd = len(sizes)
+        dx = (0.1,) * nd
+        rng = np.random.default_rng(3 + nd)
+        psi0 = wl.random_state(sizes, 1, seed=11 + nd, dx=dx)
+        w = wl.Workload("a", sizes, dx, 0.01, 1, 4, psi0, V=rng.uniform(-1, 1, size=sizes), field_kind=wl.FIELD_A,
+                        step_avg=rng.uniform(-2, 2, size=(4, nd)))
+        got, _ = gpu_steps(torch, w, 4)
+        assert rel_l2(got, oracle_steps(w, 4)) <= 1e-13
