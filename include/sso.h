@@ -70,6 +70,10 @@ extern "C" {
 #define SSO_OPT_POTENTIAL_PHASE 3        /* 0 = complex phase table exp(-i V tau/2) (default),
                                             1 = real angle table + in-kernel sincos polynomial   */
 
+#define SSO_OPT_GROUPS_PER_CTA 4         /* independent line groups per CTA (0 = auto)              */
+#define SSO_OPT_RING_BUFFERS 5           /* tile buffers of the contiguous-axis ring pipeline (0=auto) */
+#define SSO_OPT_THREADS_PER_CTA 6        /* ring pipeline CTA size: 512 (128 regs/thread) or 384 (168); 0 = auto */
+
 #define SSO_MIN_AXIS 16   /* smallest supported axis length                       */
 #define SSO_MAX_AXIS 4096 /* largest supported axis length (one CTA holds a line) */
 

@@ -37,7 +37,7 @@ template <> struct Cx2<double> { using type = double2; };
 // or, for the angle representation, the angle -V tau/2 reduced to [-pi, pi).
 template <typename T>
 __global__ void build_vtab_kernel(const double *__restrict__ V, void *__restrict__ out, long long total, int N,
-                                  const int *__restrict__ slot_nat, double half_dt, int vrep) {
+                                  const int *__restrict__ slot_nat, double half_dt, int vrep) {  // half_dt: tau/2 (half step) or tau (merged)
     using C = typename Cx2<T>::type;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
         const long long line = i / N;
@@ -96,6 +96,46 @@ __global__ void build_ephase_kernel(void *__restrict__ out, int n, const int *__
     reinterpret_cast<C *>(out)[i] = h;
 }
 
+// homogeneous E field, all passes of one sso_step call at once (2D/3D).  For every lattice axis with a field
+// component, row j of out[ax] (n[ax] complex entries) is the phase exp(-i (tau/2) c_j r) with
+//   j = 0        c = Ebar[n0]                      opening half step        (natural order)
+//   0 < j < ns   c = Ebar[n0+j-1] + Ebar[n0+j]     merged half steps        (last axis: permuted slots)
+//   j = ns       c = Ebar[n0+ns-1]                 closing half step        (natural order)
+// (eq. 11 with the step averages of reading G12; merging is PAPER.md:71 eq. 7 applied twice).
+struct ERowsArgs {
+    void *out[3];
+    int n[3];
+    double dx[3];
+    const int *slot_nat_last;
+    const double *step_avg;
+    long long n0, ns;
+    int ndim;
+    double half_dt;
+};
+template <typename T> __global__ void build_erows_kernel(const ERowsArgs e) {
+    using C = typename Cx2<T>::type;
+    const int ax = blockIdx.y;
+    if (ax >= e.ndim || !e.out[ax]) return;
+    const int n = e.n[ax];
+    const long long total = (e.ns + 1) * n;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+        const long long j = idx / n;
+        const int i = (int)(idx % n);
+        double c;
+        if (j == 0) c = e.step_avg[e.n0 * e.ndim + ax];
+        else if (j == e.ns) c = e.step_avg[(e.n0 + e.ns - 1) * e.ndim + ax];
+        else c = e.step_avg[(e.n0 + j - 1) * e.ndim + ax] + e.step_avg[(e.n0 + j) * e.ndim + ax];
+        const int nat = (ax == e.ndim - 1 && j > 0 && j < e.ns) ? e.slot_nat_last[i] : i;
+        const double r = ((double)nat - (double)(n / 2)) * e.dx[ax];
+        double sn, cs;
+        sincos(-c * e.half_dt * r, &sn, &cs);
+        C h;
+        h.x = (T)cs;
+        h.y = (T)sn;
+        reinterpret_cast<C *>(e.out[ax])[idx] = h;
+    }
+}
+
 // norm: partial sums of |psi|^2 in double, warp-shuffle tree, fixed order (deterministic)
 template <typename T>
 __global__ void norm_partial_kernel(const void *__restrict__ psi, long long count, double *__restrict__ partial) {
@@ -133,6 +173,17 @@ static LaunchFn find_launch(int precision, int N, int strided, int pw, int sign)
 #define SSO_CASE(NN) \
     case NN:         \
         return precision == SSO_C64 ? sso_lookup_f32_##NN(strided, pw, sign) : sso_lookup_f64_##NN(strided, pw, sign);
+        SSO_FOR_EACH_N(SSO_CASE)
+#undef SSO_CASE
+    }
+    return nullptr;
+}
+
+static RingLaunchFn find_ring(int precision, int N, int mode, int maxt) {
+    switch (N) {
+#define SSO_CASE(NN) \
+    case NN:         \
+        return precision == SSO_C64 ? sso_ring_lookup_f32_##NN(mode, maxt) : sso_ring_lookup_f64_##NN(mode, maxt);
         SSO_FOR_EACH_N(SSO_CASE)
 #undef SSO_CASE
     }
@@ -209,10 +260,14 @@ struct sso_plan {
     double *d_avg = nullptr;
     bool e_along_last = false;  // some row has a nonzero E component along the last axis
     long long tindex = 0;
-    void *d_vtab = nullptr;
+    void *d_vtab = nullptr;   // exp(-i V tau/2) in natural order (1D, opening and closing passes)
+    void *d_vfull = nullptr;  // exp(-i V tau) in the permuted slot order of the last axis (2D/3D steady state)
+    void *d_erow[3] = {nullptr, nullptr, nullptr};  // field phase rows of the current call (build_erows_kernel)
+    size_t erow_cap[3] = {0, 0, 0};
+    bool e_axis_on[3] = {false, false, false};
     int vrep = VREP_TABLE;
     bool kph_valid = false;
-    int opt_tl_contig = 0, opt_tl_strided = 0;
+    int opt_tl_contig = 0, opt_tl_strided = 0, opt_groups = 0, opt_ring = 0, opt_maxt = 0;
     int dbg_skip = 0;  // development only: bit 0 skip DIF, bit 1 skip DIT, bit 2 skip the pointwise factor (wrong results)
     double *d_partial = nullptr, *d_norm = nullptr;
     unsigned *d_sched = nullptr;  // tile scheduler of the pass kernel (zero between launches)
@@ -415,6 +470,8 @@ int sso_destroy(sso_plan *plan) {
     }
     cudaFree(plan->d_avg);
     cudaFree(plan->d_vtab);
+    cudaFree(plan->d_vfull);
+    for (int a = 0; a < 3; ++a) cudaFree(plan->d_erow[a]);
     cudaFree(plan->d_partial);
     cudaFree(plan->d_norm);
     cudaFree(plan->d_sched);
@@ -453,19 +510,23 @@ int sso_set_potential(sso_plan *plan, const double *V, int on_device, void *stre
     }
     const size_t entry = plan->vrep == VREP_TABLE ? plan->esize() : sizeof(double);
     cudaFree(plan->d_vtab);
-    plan->d_vtab = nullptr;
+    cudaFree(plan->d_vfull);
+    plan->d_vtab = plan->d_vfull = nullptr;
     cudaError_t e = cudaMalloc(&plan->d_vtab, entry * total);
+    if (e == cudaSuccess && plan->ndim >= 2) e = cudaMalloc(&plan->d_vfull, entry * total);
     if (e != cudaSuccess) {
         cudaFree(tmp);
         return fail(plan, SSO_ERR_ALLOC, std::string("potential table: ") + cudaGetErrorString(e));
     }
     const Axis &L = plan->ax[plan->ndim - 1];
-    const int *slot_nat = plan->ndim >= 2 ? L.d_slot_nat : nullptr;  // 1D keeps the natural order
     const int blocks = (int)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
-    if (plan->precision == SSO_C128)
-        build_vtab_kernel<double><<<blocks, 256, 0, st>>>(dV, plan->d_vtab, total, L.n, slot_nat, 0.5 * plan->dt, plan->vrep);
-    else
-        build_vtab_kernel<float><<<blocks, 256, 0, st>>>(dV, plan->d_vtab, total, L.n, slot_nat, 0.5 * plan->dt, plan->vrep);
+    if (plan->precision == SSO_C128) {
+        build_vtab_kernel<double><<<blocks, 256, 0, st>>>(dV, plan->d_vtab, total, L.n, nullptr, 0.5 * plan->dt, plan->vrep);
+        if (plan->d_vfull) build_vtab_kernel<double><<<blocks, 256, 0, st>>>(dV, plan->d_vfull, total, L.n, L.d_slot_nat, plan->dt, plan->vrep);
+    } else {
+        build_vtab_kernel<float><<<blocks, 256, 0, st>>>(dV, plan->d_vtab, total, L.n, nullptr, 0.5 * plan->dt, plan->vrep);
+        if (plan->d_vfull) build_vtab_kernel<float><<<blocks, 256, 0, st>>>(dV, plan->d_vfull, total, L.n, L.d_slot_nat, plan->dt, plan->vrep);
+    }
     e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     cudaFree(tmp);
@@ -483,6 +544,7 @@ int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nval
         cudaFree(plan->d_avg);
         plan->d_avg = nullptr;
         plan->e_along_last = false;
+        for (int a = 0; a < 3; ++a) plan->e_axis_on[a] = false;
         plan->kph_valid = false;
         return SSO_OK;
     }
@@ -503,9 +565,31 @@ int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nval
     plan->nvals = nvals;
     plan->field_kind = kind;
     plan->e_along_last = false;
+    for (int a = 0; a < 3; ++a) plan->e_axis_on[a] = false;
     if (kind == SSO_FIELD_E)
         for (int64_t n = 0; n < nvals; ++n)
-            if (step_avg[n * plan->ndim + plan->ndim - 1] != 0.0) plan->e_along_last = true;
+            for (int a = 0; a < plan->ndim; ++a)
+                if (step_avg[n * plan->ndim + a] != 0.0) plan->e_axis_on[a] = true;
+    plan->e_along_last = plan->e_axis_on[plan->ndim - 1];
+    // phase rows of one call (2D/3D): allocated here so that sso_step only enqueues kernels
+    if (kind == SSO_FIELD_E && plan->ndim >= 2) {
+        int nmax = 16;
+        for (int a = 0; a < plan->ndim; ++a)
+            if (plan->e_axis_on[a] && plan->ax[a].n > nmax) nmax = plan->ax[a].n;
+        long long chunk = (64LL << 20) / ((long long)nmax * (long long)plan->esize()) - 1;
+        if (chunk < 1) chunk = 1;
+        const long long rows = (nvals < chunk ? nvals : chunk) + 1;
+        for (int a = 0; a < plan->ndim; ++a) {
+            cudaFree(plan->d_erow[a]);
+            plan->d_erow[a] = nullptr;
+            plan->erow_cap[a] = 0;
+            if (!plan->e_axis_on[a]) continue;
+            const size_t need = (size_t)rows * plan->ax[a].n * plan->esize();
+            cudaError_t ce = cudaMalloc(&plan->d_erow[a], need);
+            if (ce != cudaSuccess) return fail(plan, SSO_ERR_ALLOC, std::string("field phase rows: ") + cudaGetErrorString(ce));
+            plan->erow_cap[a] = need;
+        }
+    }
     plan->kph_valid = false;
     return SSO_OK;
 }
@@ -533,6 +617,18 @@ int sso_set_option(sso_plan *plan, int option, int64_t value) {
             return SSO_OK;
         case 100:
             plan->dbg_skip = (int)value;
+            return SSO_OK;
+        case SSO_OPT_RING_BUFFERS:
+            if (value < 0 || value > 16) return fail(plan, SSO_ERR_INVALID, "ring buffers must be in [0, 16]");
+            plan->opt_ring = (int)value;
+            return SSO_OK;
+        case SSO_OPT_THREADS_PER_CTA:
+            if (value != 0 && value != 384 && value != 512) return fail(plan, SSO_ERR_INVALID, "threads per CTA must be 0, 384 or 512");
+            plan->opt_maxt = (int)value;
+            return SSO_OK;
+        case SSO_OPT_GROUPS_PER_CTA:
+            if (value < 0 || value > 15) return fail(plan, SSO_ERR_INVALID, "groups per CTA must be in [0, 15]");
+            plan->opt_groups = (int)value;
             return SSO_OK;
         case SSO_OPT_POTENTIAL_PHASE:
             if (value != VREP_TABLE && value != VREP_ANGLE) return fail(plan, SSO_ERR_INVALID, "potential phase mode must be 0 or 1");
@@ -647,6 +743,7 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
     a.unpermute = s.unpermute;
     a.mid_on = (plan->dbg_skip & 4) ? 0 : s.mid_on;
     a.dbg_copy = (plan->dbg_skip & 8) ? 1 : 0;
+    a.dbg_flags = (plan->dbg_skip >> 6) & 3;
     a.pre_v = s.pre_v;
     a.post_v = s.post_v;
     a.nrep = s.nrep;
@@ -695,12 +792,136 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
     if (work > 0x7fffffffLL) return fail(plan, SSO_ERR_UNSUPPORTED, "too many tiles");
     a.ntiles = (int)work;
     a.sched = plan->d_sched;
-    const unsigned threads = (unsigned)(cc * TL * U);
-    size_t smem = (size_t)twiddle_count_padded(A.n) * esz + (size_t)cc * TL * pitch * esz + (size_t)TL * esz + 2 * sizeof(int);
-    smem = (smem + 127) & ~(size_t)127;
+    // groups per CTA: independent pipelines (own exchange buffer and barrier) that share one twiddle copy.
+    // As many as fit in 512 threads (complex128: 128 registers/thread) or 1024 (complex64) and in shared memory.
+    const int GT = cc * TL * U;
+    size_t greg = (size_t)cc * TL * pitch * esz + (size_t)TL * esz + 2 * sizeof(int);
+    greg = (greg + 127) & ~(size_t)127;
+    const size_t twbytes = (size_t)twiddle_count_padded(A.n) * esz;
+    int G = 1;
+    if (GT % 32 == 0) {
+        const int maxthreads = 512;
+        G = plan->opt_groups > 0 ? plan->opt_groups : maxthreads / GT;
+        while (G > 1 && ((size_t)G * greg + twbytes > 227 * 1024 - 1024 || G * GT > maxthreads)) --G;
+        if (G > 15) G = 15;
+        if (G < 1) G = 1;
+        const long long tiles_per_sm = (work + 147) / 148;
+        if (G > tiles_per_sm) G = (int)(tiles_per_sm > 0 ? tiles_per_sm : 1);
+    }
+    a.G = G;
+    a.GT = GT;
+    a.gstride = (int)(greg / esz);
+    const unsigned threads = (unsigned)(G * GT);
+    size_t smem = twbytes + (size_t)G * greg;
+    if ((plan->dbg_skip >> 8) & 1) smem = smem < 120 * 1024 ? 120 * 1024 : smem;  // development: one CTA per SM
     cudaError_t e = fn(a, threads, smem, st);
     if (e != cudaSuccess) return cuda_fail(plan, e, "pass kernel launch");
     return SSO_OK;
+}
+
+
+// contiguous-axis pass of a 2D/3D lattice through the ring pipeline (sso_ring.cuh).  `row` selects the field
+// phase row of this call (build_erows_kernel): 0 opening, j merged after step j-1, nsteps closing.
+int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStream_t st) {
+    const int last = plan->ndim - 1;
+    const Axis &A = plan->ax[last];
+    const int U = A.n / 16;
+    const int esz = (int)plan->esize();
+    const long long lines = plan->npts / A.n;       // per component
+    // group tile: 128 threads = 2048 points (fewer when the lattice has fewer lines)
+    int TL = plan->opt_tl_contig > 0 ? plan->opt_tl_contig : (U >= 128 ? 1 : 128 / U);
+    while (TL > 1 && (lines % TL != 0 || TL * U > 512)) TL /= 2;
+    const int GT = TL * U;
+    const int pitch = A.n + A.n / 16;
+    size_t bufbytes = (size_t)TL * pitch * esz;
+    bufbytes = (bufbytes + 127) & ~(size_t)127;
+    const size_t twbytes = (size_t)twiddle_count_padded(A.n) * esz;
+    const long long ntiles = lines * plan->ncomp / TL;
+    if (ntiles > 0x7fffffffLL) return fail(plan, SSO_ERR_UNSUPPORTED, "too many tiles");
+    const int maxt = plan->opt_maxt == 384 ? 384 : 512;
+    int G = 1;
+    if (GT % 32 == 0) {
+        G = plan->opt_groups > 0 ? plan->opt_groups : maxt / GT;
+        while (G > 1 && G * GT > maxt) --G;
+        if (G > 15) G = 15;
+        const long long per_sm = (ntiles + 147) / 148;
+        if (G > per_sm) G = (int)per_sm;
+        if (G < 1) G = 1;
+    }
+    const size_t avail = 227 * 1024 - 256 - twbytes;
+    int NB = (int)(avail / bufbytes);
+    const int want = plan->opt_ring > 0 ? plan->opt_ring : G + 2 + G / 2;
+    if (NB > want) NB = want;
+    if (NB > 16) NB = 16;
+    if (NB < 1) return fail(plan, SSO_ERR_UNSUPPORTED, "line too long for the ring pipeline");
+    if (G > NB) G = NB;
+    RingArgs a{};
+    a.psi = psi;
+    a.tw = A.tw;
+    a.revB = A.d_revB;
+    a.ntiles = (int)ntiles;
+    a.TL = TL;
+    a.pitch = pitch;
+    a.G = G;
+    a.GT = GT;
+    a.NB = NB;
+    a.bufstride = (int)(bufbytes / esz);
+    a.lines_per_comp = (int)lines;
+    const Geometry g = geometry(plan, last);
+    a.rest1 = g.rest1;
+    a.vtab = mode == MODE_MID ? plan->d_vfull : plan->d_vtab;
+    a.vrep = plan->vrep;
+    if (plan->field_kind == SSO_FIELD_E) {
+        if (plan->e_axis_on[last]) a.eline = (const char *)plan->d_erow[last] + (size_t)row * A.n * esz;
+        if (g.oaxA >= 0 && plan->e_axis_on[g.oaxA]) a.eoA = (const char *)plan->d_erow[g.oaxA] + (size_t)row * plan->ax[g.oaxA].n * esz;
+        if (g.oaxB >= 0 && plan->e_axis_on[g.oaxB]) a.eoB = (const char *)plan->d_erow[g.oaxB] + (size_t)row * plan->ax[g.oaxB].n * esz;
+    }
+    RingLaunchFn fn = find_ring(plan->precision, A.n, mode, maxt);
+    if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no ring kernel built for this line length");
+    const size_t smem = twbytes + (size_t)NB * bufbytes + (size_t)NB * 8;
+    const unsigned grid = (unsigned)(ntiles < 148 ? ntiles : 148);
+    cudaError_t e = fn(a, (unsigned)(G * GT), smem, grid, st);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "ring kernel launch");
+    return SSO_OK;
+}
+
+// field phase rows for steps [n0, n0 + ns) of a 2D/3D call
+int build_erows(sso_plan *plan, long long n0, long long ns, cudaStream_t st) {
+    if (plan->field_kind != SSO_FIELD_E) return SSO_OK;
+    ERowsArgs e{};
+    bool any = false;
+    for (int a = 0; a < plan->ndim; ++a) {
+        e.n[a] = plan->ax[a].n;
+        e.dx[a] = plan->ax[a].dx;
+        if (!plan->e_axis_on[a]) continue;
+        const size_t need = (size_t)(ns + 1) * plan->ax[a].n * plan->esize();
+        if (need > plan->erow_cap[a]) return fail(plan, SSO_ERR_STATE, "field phase rows not allocated (sso_set_field allocates them)");
+        e.out[a] = plan->d_erow[a];
+        any = true;
+    }
+    if (!any) return SSO_OK;
+    e.slot_nat_last = plan->ax[plan->ndim - 1].d_slot_nat;
+    e.step_avg = plan->d_avg;
+    e.n0 = n0;
+    e.ns = ns;
+    e.ndim = plan->ndim;
+    e.half_dt = 0.5 * plan->dt;
+    dim3 grid(64, plan->ndim);
+    if (plan->precision == SSO_C128) build_erows_kernel<double><<<grid, 256, 0, st>>>(e);
+    else build_erows_kernel<float><<<grid, 256, 0, st>>>(e);
+    cudaError_t ce = cudaGetLastError();
+    if (ce != cudaSuccess) return cuda_fail(plan, ce, "field phase rows kernel");
+    return SSO_OK;
+}
+
+// steps of one 2D/3D call small enough for one set of field phase rows
+long long erow_chunk(const sso_plan *p) {
+    if (p->field_kind != SSO_FIELD_E) return 0x7fffffffffffLL;
+    int nmax = 16;
+    for (int a = 0; a < p->ndim; ++a)
+        if (p->e_axis_on[a] && p->ax[a].n > nmax) nmax = p->ax[a].n;
+    const long long c = (64LL << 20) / ((long long)nmax * (long long)p->esize()) - 1;
+    return c < 1 ? 1 : c;
 }
 
 // (re)build the Schroedinger kinetic phase tables; with SSO_FIELD_A they depend on the step
@@ -733,10 +954,13 @@ long long launches_for(const sso_plan *p, long long nsteps) {
         if (kshift) return nsteps * (1 + p->ndim);
         return 1 + (kbuild ? p->ndim : 0);
     }
-    const bool eph = p->field_kind == SSO_FIELD_E && p->e_along_last;
-    cnt += 1;                                    // opening
+    const long long chunk = erow_chunk(p);
+    const long long nchunks = (nsteps + chunk - 1) / chunk;
+    bool eph = false;
+    for (int a = 0; a < p->ndim; ++a) eph = eph || (p->field_kind == SSO_FIELD_E && p->e_axis_on[a]);
+    cnt += nchunks * (eph ? 2 : 1);              // opening pass (+ field phase rows)
     cnt += nsteps * (p->ndim == 3 ? 3 : 1);      // kinetic sandwich (+ middle-axis DIF and DIT)
-    cnt += nsteps * (eph ? 2 : 1);               // potential sandwiches and the closing pass
+    cnt += nsteps;                               // potential sandwiches and the closing pass
     if (kshift) cnt += nsteps * p->ndim;
     else if (kbuild) cnt += p->ndim;
     return cnt;
@@ -776,29 +1000,29 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
             if ((rc = launch(plan, psi, ps, st)) != SSO_OK) return rc;
         }
     } else {
-        const int last = nd - 1;
-        // opening: V/2 in natural order, forward transform along the last axis, natural frequency order out
-        PassSpec open{last, PW_NONE, -1, 1, 0, 1, 0, 2, 0, 0, 1, n0};
-        if ((rc = launch(plan, psi, open, st)) != SSO_OK) return rc;
-        for (long long s = 0; s < nsteps; ++s) {
-            const long long n = n0 + s;
-            if (plan->ncomp == 1 && (rc = build_kphase(plan, n, st)) != SSO_OK) return rc;
-            if (nd == 3) {
-                PassSpec mid{1, PW_NONE, -1, 1, 0, 0, 0, 0, 0, 0, 1, n};  // F_1, stored in network order
-                if ((rc = launch(plan, psi, mid, st)) != SSO_OK) return rc;
-            }
-            PassSpec kin{0, kpw, -1, 1, 1, 0, 1, 0, 0, 0, 1, n};  // F_0 K F_0^-1
-            if ((rc = launch(plan, psi, kin, st)) != SSO_OK) return rc;
-            if (nd == 3) {
-                PassSpec mid{1, PW_NONE, -1, 0, 1, 0, 0, 0, 0, 0, 1, n};  // F_1^-1 from network order
-                if ((rc = launch(plan, psi, mid, st)) != SSO_OK) return rc;
-            }
-            if (s + 1 < nsteps) {
-                PassSpec pot{last, PW_V, +1, 1, 1, 0, 1, 0, 0, 1, 1, n};  // F_last^-1 V(n, n+1) F_last
-                if ((rc = launch(plan, psi, pot, st)) != SSO_OK) return rc;
-            } else {
-                PassSpec close{last, PW_V, +1, 1, 0, 1, 1, 0, 0, 0, 1, n};  // F_last^-1, V/2, natural order out
-                if ((rc = launch(plan, psi, close, st)) != SSO_OK) return rc;
+        // chunks that share one set of field phase rows; each chunk opens and closes with a half step
+        const long long chunk = erow_chunk(plan);
+        for (long long c0 = 0; c0 < nsteps; c0 += chunk) {
+            const long long ns = nsteps - c0 < chunk ? nsteps - c0 : chunk;
+            const long long nb = n0 + c0;
+            if ((rc = build_erows(plan, nb, ns, st)) != SSO_OK) return rc;
+            // opening: V/2 in natural order, forward transform along the last axis, natural frequency order out
+            if ((rc = launch_ring_pass(plan, psi, MODE_OPEN, 0, st)) != SSO_OK) return rc;
+            for (long long s = 0; s < ns; ++s) {
+                const long long n = nb + s;
+                if (plan->ncomp == 1 && (rc = build_kphase(plan, n, st)) != SSO_OK) return rc;
+                if (nd == 3) {
+                    PassSpec mid{1, PW_NONE, -1, 1, 0, 0, 0, 0, 0, 0, 1, n};  // F_1, stored in network order
+                    if ((rc = launch(plan, psi, mid, st)) != SSO_OK) return rc;
+                }
+                PassSpec kin{0, kpw, -1, 1, 1, 0, 1, 0, 0, 0, 1, n};  // F_0 K F_0^-1
+                if ((rc = launch(plan, psi, kin, st)) != SSO_OK) return rc;
+                if (nd == 3) {
+                    PassSpec mid{1, PW_NONE, -1, 0, 1, 0, 0, 0, 0, 0, 1, n};  // F_1^-1 from network order
+                    if ((rc = launch(plan, psi, mid, st)) != SSO_OK) return rc;
+                }
+                // F_last^-1 V(n, n+1) F_last, or the closing F_last^-1, V/2
+                if ((rc = launch_ring_pass(plan, psi, s + 1 < ns ? MODE_MID : MODE_CLOSE, s + 1, st)) != SSO_OK) return rc;
             }
         }
     }

@@ -23,10 +23,13 @@ struct PassArgs {
     int ncomp;               // components in psi
     int TL;                  // lines per component per CTA
     int pitch;               // shared-memory line pitch in complex elements
+    int G, GT;               // groups per CTA (independent pipelines sharing the twiddle table), threads per group
+    int gstride;             // complex elements between the shared-memory regions of consecutive groups
     int rest1;               // size of the faster non-line axis: line index = ia * rest1 + ib, >= 1
     int oaxA, oaxB;          // lattice axes that ia and ib run along (-1: absent)
     // structure of the pass
     int do_dif, do_dit, unpermute;
+    int dbg_flags;           // development only: bit 0 no table prefetch, bit 1 no next-tile prefetch
     int dbg_copy;            // development only: load and store in the coalesced layout, nothing in between
     int mid_on;              // apply the pointwise factor between DIF and DIT
     int pre_v, post_v;       // 0 none; 1 natural-order table (1D); 2 gather from the permuted table (opening pass)
@@ -67,5 +70,33 @@ using LaunchFn = cudaError_t (*)(const PassArgs &, unsigned threads, size_t smem
     LaunchFn sso_lookup_f64_##N(int strided, int pw, int sign);
 SSO_FOR_EACH_N(SSO_DECL_LOOKUP)
 #undef SSO_DECL_LOOKUP
+
+// the ring pipeline of sso_ring.cuh (contiguous-axis passes of 2D/3D lattices)
+enum : int { MODE_OPEN = 0, MODE_MID = 1, MODE_CLOSE = 2 };
+
+struct RingArgs {
+    void *psi;                // device, all components: ntiles * TL lines of N points, contiguous
+    const void *tw;           // twiddle blocks of this axis (as in PassArgs)
+    const int *revB;          // int[N/16]
+    int ntiles;               // tiles of TL lines over all components
+    int TL;                   // lines per tile
+    int pitch;                // padded line pitch (complex elements) of the exchange layout
+    int G, GT;                // groups per CTA, threads per group (= TL * N/16)
+    int NB;                   // ring buffers
+    int bufstride;            // complex elements between ring buffers
+    int lines_per_comp;       // lines of one component (the potential table repeats per component)
+    int rest1;                // table line = ia * rest1 + ib
+    const void *vtab;         // MODE_MID: merged phase exp(-i V tau), permuted slots; else exp(-i V tau/2), natural
+    int vrep;                 // VREP_TABLE (complex phases) or VREP_ANGLE (real angles, sincos in the kernel)
+    const void *eline;        // complex[N] field phase along the line for this pass (same order as vtab) or NULL
+    const void *eoA, *eoB;    // complex field phase rows of the other axes, indexed by ia / ib, or NULL
+};
+
+using RingLaunchFn = cudaError_t (*)(const RingArgs &, unsigned threads, size_t smem, unsigned grid, cudaStream_t st);
+#define SSO_DECL_RING(N)                                  \
+    RingLaunchFn sso_ring_lookup_f32_##N(int mode, int maxt); \
+    RingLaunchFn sso_ring_lookup_f64_##N(int mode, int maxt);
+SSO_FOR_EACH_N(SSO_DECL_RING)
+#undef SSO_DECL_RING
 
 }  // namespace sso

@@ -3,6 +3,7 @@
 // (see paper_1012_3911_b200/build.py); each object exports one lookup function that the
 // dispatcher in sso_api.cu calls.
 #include "sso_pass.cuh"
+#include "sso_ring.cuh"
 #include "sso_dispatch.h"
 
 #ifndef SSO_T
@@ -42,13 +43,49 @@ cudaError_t launch_pass(const PassArgs &a, unsigned threads, size_t smem, cudaSt
         key_occ[slot] = occ;
     }
     long long grid = (long long)occ * num_sms;
-    if (grid > a.ntiles) grid = a.ntiles;
+    const long long need = ((long long)a.ntiles + a.G - 1) / a.G;
+    if (grid > need) grid = need;
     kern<<<(unsigned)grid, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <typename T, int N, int MODE, int SIGN, int MAXT>
+cudaError_t launch_ring(const RingArgs &a, unsigned threads, size_t smem, unsigned grid, cudaStream_t st) {
+    auto kern = ring_kernel<T, N, MODE, SIGN, MAXT>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    if (threads > (unsigned)MAXT) return cudaErrorInvalidConfiguration;
+    kern<<<grid, threads, smem, st>>>(a);
     return cudaGetLastError();
 }
 
 #define SSO_CAT3_(a, b, c) a##b##_##c
 #define SSO_CAT3(a, b, c) SSO_CAT3_(a, b, c)
+
+#define SSO_CAT4_(a, b, c) a##b##_##c
+#define SSO_CAT4(a, b, c) SSO_CAT4_(a, b, c)
+#ifdef SSO_STUB
+RingLaunchFn SSO_CAT4(sso_ring_lookup_, SSO_TNAME, SSO_N)(int, int) { return nullptr; }
+#else
+RingLaunchFn SSO_CAT4(sso_ring_lookup_, SSO_TNAME, SSO_N)(int mode, int maxt) {
+    using T = SSO_T;
+    constexpr int N = SSO_N;
+    if (maxt == 512) {
+        if (mode == MODE_OPEN) return &launch_ring<T, N, MODE_OPEN, -1, 512>;
+        if (mode == MODE_MID) return &launch_ring<T, N, MODE_MID, +1, 512>;
+        if (mode == MODE_CLOSE) return &launch_ring<T, N, MODE_CLOSE, +1, 512>;
+    } else if (maxt == 384) {
+        if (mode == MODE_OPEN) return &launch_ring<T, N, MODE_OPEN, -1, 384>;
+        if (mode == MODE_MID) return &launch_ring<T, N, MODE_MID, +1, 384>;
+        if (mode == MODE_CLOSE) return &launch_ring<T, N, MODE_CLOSE, +1, 384>;
+    }
+    return nullptr;
+}
+#endif
 
 #ifdef SSO_STUB
 // development builds may leave a size out (SSO_SIZES in build.py): the dispatcher then reports "unsupported"

@@ -229,36 +229,43 @@ template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void di
     for (int s = 0; s < S; ++s) dft_reg<R, S, SIGN>(&x[s]);
 }
 
+// barrier over one group of a CTA (groups are independent pipelines that share only the twiddle table):
+// gb = 0 means the CTA holds one group (plain __syncthreads), otherwise gb = (named barrier id) | (threads << 8)
+__device__ __forceinline__ void gsync(int gb) {
+    if (gb == 0) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(gb & 15), "r"(gb >> 8) : "memory");
+}
+
 // registers (layout of stage IA) -> shared memory -> registers (layout of stage IB)
-template <typename T, int N, int IA, int IB> __device__ __forceinline__ void exchange(typename CxOf<T>::type (&x)[16], int u, typename CxOf<T>::type *sl) {
+template <typename T, int N, int IA, int IB> __device__ __forceinline__ void exchange(typename CxOf<T>::type (&x)[16], int u, typename CxOf<T>::type *sl, int gb) {
     using C = typename CxOf<T>::type;
     C *wa = sl + stage_base<N, IA>(u);
     const C *rb = sl + stage_base<N, IB>(u);
-    __syncthreads();
+    gsync(gb);
 #pragma unroll
     for (int q = 0; q < 16; ++q) wa[stage_delta<N, IA>(q)] = x[q];
-    __syncthreads();
+    gsync(gb);
 #pragma unroll
     for (int q = 0; q < 16; ++q) x[q] = rb[stage_delta<N, IB>(q)];
 }
 
 template <typename T, int N, int I, int SIGN> struct DifChain {
     using C = typename CxOf<T>::type;
-    static __device__ __forceinline__ void run(C (&x)[16], int u, const C *tw, C *sl) {
+    static __device__ __forceinline__ void run(C (&x)[16], int u, const C *tw, C *sl, int gb) {
         dif_stage<T, N, I, SIGN>(x, u, tw);
         if constexpr (I + 1 < Sched<N>::M) {
-            exchange<T, N, I, I + 1>(x, u, sl);
-            DifChain<T, N, I + 1, SIGN>::run(x, u, tw, sl);
+            exchange<T, N, I, I + 1>(x, u, sl, gb);
+            DifChain<T, N, I + 1, SIGN>::run(x, u, tw, sl, gb);
         }
     }
 };
 template <typename T, int N, int I, int SIGN> struct DitChain {  // runs stages I, I-1, ..., 0
     using C = typename CxOf<T>::type;
-    static __device__ __forceinline__ void run(C (&x)[16], int u, const C *tw, C *sl) {
+    static __device__ __forceinline__ void run(C (&x)[16], int u, const C *tw, C *sl, int gb) {
         dit_stage<T, N, I, SIGN>(x, u, tw);
         if constexpr (I > 0) {
-            exchange<T, N, I, I - 1>(x, u, sl);
-            DitChain<T, N, I - 1, SIGN>::run(x, u, tw, sl);
+            exchange<T, N, I, I - 1>(x, u, sl, gb);
+            DitChain<T, N, I - 1, SIGN>::run(x, u, tw, sl, gb);
         }
     }
 };
@@ -302,7 +309,12 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
     C *sm = stw + TWP;
 
     const int TL = a.TL;
-    const int tid = threadIdx.x;
+    // groups: G independent pipelines of GT = CC * TL * U threads each; a group owns an exchange buffer,
+    // its per-line scalars and its scheduler mailbox, and synchronises with its own named barrier
+    const int GT = a.GT;
+    const int grp = threadIdx.x / GT;
+    const int tid = threadIdx.x - grp * GT;
+    const int gb = a.G > 1 ? ((grp + 1) | (GT << 8)) : 0;
     int t, c, u;
     if (STRIDED) {
         t = tid % TL;
@@ -315,14 +327,15 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
         t = ct % TL;
         c = ct / TL;
     }
-    C *sl = sm + (c * TL + t) * a.pitch;
-    C *lsc = sm + CC * TL * a.pitch;                       // per-line scalars [TL] (complex)
+    C *smg = sm + (size_t)grp * a.gstride;                  // this group's region
+    C *sl = smg + (c * TL + t) * a.pitch;
+    C *lsc = smg + CC * TL * a.pitch;                       // per-line scalars [TL] (complex)
     int *snext = reinterpret_cast<int *>(lsc + TL);         // tile scheduler mailbox [2]
 
     // twiddles -> shared memory, once per CTA
     {
         const C *__restrict__ gtw = reinterpret_cast<const C *>(a.tw);
-        for (int i = tid; i < TWN; i += blockDim.x) stw[i] = gtw[i];
+        for (int i = threadIdx.x; i < TWN; i += blockDim.x) stw[i] = gtw[i];
     }
     if (tid == 0) snext[0] = (int)atomicAdd(&a.sched[0], 1u);
     __syncthreads();
@@ -377,7 +390,7 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
             for (int q = 0; q < 16; ++q) x[q] = ld_stream(&gp[(long long)(u * 16 + q) * estep]);
         }
         if constexpr (PW == PW_V) {
-            if (a.mid_on && u == 0) {
+            if (a.mid_on && u == 0 && !(a.dbg_flags & 1)) {
                 const size_t esz = a.vrep == VREP_TABLE ? sizeof(C) : sizeof(double);
                 prefetch_l2_bulk(reinterpret_cast<const char *>(a.vtab) + (size_t)line * N * esz, (unsigned)(N * esz));
             }
@@ -433,9 +446,9 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
         };
 
         // every thread learns the next tile and asks L2 for its share of that tile
-        __syncthreads();  // also orders the twiddle copy (first tile) and lsc before their use
+        gsync(gb);  // also orders the twiddle copy (first tile) and lsc before their use
         const int ntile = snext[parity];
-        if (ntile < a.ntiles) {
+        if (ntile < a.ntiles && !(a.dbg_flags & 2)) {
             long long tile2 = CC == 1 ? ntile / a.ncomp : ntile;
             const int comp2 = CC == 1 ? ntile % a.ncomp : c;
             const long long line2 = tile2 * TL + t;
@@ -465,14 +478,14 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
             const long long n = a.n0 + rep;
             if (a.pre_v && rep == 0) natural_v(a.pre_v, n, n, false);
 
-            if (a.do_dif) DifChain<T, N, 0, SIGN>::run(x, u, stw, sl);
+            if (a.do_dif) DifChain<T, N, 0, SIGN>::run(x, u, stw, sl, gb);
 
             if (a.mid_on) {
                 if constexpr (PW == PW_V) {
                     // merged or half potential phase in the permuted order: register q of thread u is
                     // table slot q U + u (coalesced across u)
                     if (a.field_kind == 1 && u == 0) lsc[t] = expi<T>(-other_axes_angle(n, n + 1, a.v_mid_full != 0));
-                    if (a.field_kind == 1) __syncthreads();
+                    if (a.field_kind == 1) gsync(gb);
                     const long long vb = line * (long long)N + u;
 #pragma unroll
                     for (int q = 0; q < 16; ++q) {
@@ -513,15 +526,15 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
                     // all components of a k point into one thread: thread (c, u) takes the PP points
                     // 16 u + c PP + i of every component
                     C *me = sl + 17 * u;
-                    __syncthreads();
+                    gsync(gb);
 #pragma unroll
                     for (int q = 0; q < 16; ++q) me[q] = x[q];
-                    __syncthreads();
+                    gsync(gb);
                     C y[CC][PP];
 #pragma unroll
                     for (int c2 = 0; c2 < CC; ++c2)
 #pragma unroll
-                        for (int i = 0; i < PP; ++i) y[c2][i] = sm[(c2 * TL + t) * a.pitch + 17 * u + c * PP + i];
+                        for (int i = 0; i < PP; ++i) y[c2][i] = smg[(c2 * TL + t) * a.pitch + 17 * u + c * PP + i];
                     const double mc2 = a.mass * a.clight * a.clight;
 #pragma unroll
                     for (int i = 0; i < PP; ++i) {
@@ -562,14 +575,14 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
 #pragma unroll
                     for (int c2 = 0; c2 < CC; ++c2)
 #pragma unroll
-                        for (int i = 0; i < PP; ++i) sm[(c2 * TL + t) * a.pitch + 17 * u + c * PP + i] = y[c2][i];
-                    __syncthreads();
+                        for (int i = 0; i < PP; ++i) smg[(c2 * TL + t) * a.pitch + 17 * u + c * PP + i] = y[c2][i];
+                    gsync(gb);
 #pragma unroll
                     for (int q = 0; q < 16; ++q) x[q] = me[q];
                 }
             }
 
-            if (a.do_dit) DitChain<T, N, LAST, -SIGN>::run(x, u, stw, sl);
+            if (a.do_dit) DitChain<T, N, LAST, -SIGN>::run(x, u, stw, sl, gb);
 
             if (a.post_v) {
                 if (rep + 1 < a.nrep) natural_v(a.post_v, n, n + 1, true);
@@ -581,10 +594,10 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
             // registers hold frequency revB[u] + U q at position 16 u + q: scatter to natural order
             C *wa = sl + padp(a.revB[u]);
             const C *rb = sl + padp(u);
-            __syncthreads();
+            gsync(gb);
 #pragma unroll
             for (int q = 0; q < 16; ++q) wa[lin_delta(q, U)] = x[q];
-            __syncthreads();
+            gsync(gb);
 #pragma unroll
             for (int q = 0; q < 16; ++q) x[q] = rb[lin_delta(q, U)];
         }
@@ -598,11 +611,12 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
 
         wtile = ntile;
         parity ^= 1;
-        __syncthreads();  // everyone is done with the exchange buffer, lsc and the mailbox slot
+        gsync(gb);  // everyone is done with the exchange buffer, lsc and the mailbox slot
     }
 
     // the last CTA to leave resets the scheduler for the next launch on this stream
-    if (tid == 0) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
         __threadfence();
         const unsigned done = atomicAdd(&a.sched[1], 1u);
         if (done == gridDim.x - 1) {

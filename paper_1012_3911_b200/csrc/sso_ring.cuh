@@ -1,0 +1,220 @@
+// sso_ring.cuh -- the contiguous-axis pass of a 2D/3D lattice as an asynchronous ring pipeline (sm_100a).
+//
+// The last lattice axis is contiguous in memory, so a tile of TL whole lines is one contiguous block.  One
+// persistent CTA per SM owns a ring of NB shared-memory buffers.  Tiles are moved by the bulk-copy engine
+// (cp.async.bulk, SASS UBLKCP): global -> buffer, completion signalled on an mbarrier, and buffer -> global
+// as a bulk store.  G independent groups of GT threads each take the tiles of the ring in turn, and, with the
+// tile in registers (16 points per thread) and its buffer as the exchange area, apply
+//
+//   MODE_OPEN   V/2 (natural order)  ->  forward DIF  ->  natural frequency order
+//   MODE_MID    inverse DIF  ->  merged potential phase V (permuted order)  ->  forward DIT
+//   MODE_CLOSE  inverse DIF  ->  natural order  ->  V/2
+//
+// (eq. 7, 98 eq. 11; the FFT stages are those of sso_pass.cuh).  No thread ever waits for HBM
+// with work in its registers: the load of the tile that will reuse a buffer is issued as soon as that
+// buffer's store has been read out, NB tiles ahead of its use, and the potential-phase lines of that tile
+// are requested into L2 at the same time.
+#pragma once
+#include "sso_pass.cuh"
+
+namespace sso {
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(void *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void *bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P, [%0], %1;\n"
+        "@P bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_load(void *smem_dst, const void *gsrc, unsigned bytes, void *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_store(void *gdst, const void *smem_src, unsigned bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// streamed table loads: read once per pass, so keep them out of L1 and first in line for eviction from L2
+// (psi of the L2-sized configs then stays resident between passes)
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ double2 ld_table(const double2 *p, uint64_t pol) {
+    double2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ float2 ld_table(const float2 *p, uint64_t pol) {
+    float2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double ld_table(const double *p, uint64_t pol) {
+    double v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ void prefetch_l2_bulk_hint(const void *p, unsigned bytes, uint64_t pol) {
+    asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(p), "r"(bytes), "l"(pol) : "memory");
+}
+
+template <typename T, int N, int MODE, int SIGN, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
+    using C = typename CxOf<T>::type;
+    constexpr int U = N / 16;
+    constexpr int LAST = Sched<N>::M - 1;
+    constexpr int TWN = Sched<N>::twoff(LAST);
+    constexpr int TWP = (TWN + 7) & ~7;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    C *stw = reinterpret_cast<C *>(smem_raw);
+    C *bufs = stw + TWP;
+    unsigned long long *full = reinterpret_cast<unsigned long long *>(bufs + (size_t)a.NB * a.bufstride);
+
+    const int TL = a.TL, GT = a.GT, G = a.G, NB = a.NB;
+    const int grp = threadIdx.x / GT;
+    const int tid = threadIdx.x - grp * GT;
+    const int gb = G > 1 ? ((grp + 1) | (GT << 8)) : 0;
+    const int u = tid % U;
+    const int t = tid / U;
+    const unsigned tile_bytes = (unsigned)(TL * N * sizeof(C));
+    const int nloc = a.ntiles > (int)blockIdx.x ? (a.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    const uint64_t pol = policy_evict_first();
+    const size_t vesz = a.vrep == VREP_TABLE ? sizeof(C) : sizeof(double);
+    C *gpsi = reinterpret_cast<C *>(a.psi);
+
+    // issue the load of local tile k into its ring buffer, and ask L2 for that tile's potential-phase lines
+    auto issue = [&](int k) {
+        const int b = k % NB;
+        const long long tile = (long long)blockIdx.x + (long long)k * gridDim.x;
+        mbar_expect_tx(&full[b], tile_bytes);
+        bulk_load(bufs + (size_t)b * a.bufstride, gpsi + tile * TL * N, tile_bytes, &full[b]);
+        if (a.vtab) {
+            const long long l0 = (tile * TL) % a.lines_per_comp;  // a tile never straddles two components
+            prefetch_l2_bulk_hint(reinterpret_cast<const char *>(a.vtab) + (size_t)l0 * N * vesz, (unsigned)(TL * N * vesz), pol);
+        }
+    };
+
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < NB; ++b) mbar_init(&full[b], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    {
+        const C *__restrict__ gtw = reinterpret_cast<const C *>(a.tw);
+        for (int i = threadIdx.x; i < TWN; i += blockDim.x) stw[i] = gtw[i];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0)
+        for (int k = 0; k < NB && k < nloc; ++k) issue(k);
+
+    for (int k = grp; k < nloc; k += G) {
+        const int b = k % NB;
+        C *buf = bufs + (size_t)b * a.bufstride;
+        C *dense = buf + t * N + u;          // bulk-copy layout: [TL][N]
+        C *sl = buf + t * a.pitch;           // exchange layout: padded lines
+        const long long tile = (long long)blockIdx.x + (long long)k * gridDim.x;
+        const int lic = (int)((tile * TL + t) % a.lines_per_comp);  // line within the component = table line
+        const size_t vbase = (size_t)lic * N + u;
+
+        // pointwise factor of this pass for register q (table slot q U + u of line lic)
+        auto phase = [&](C (&x)[16]) {
+            C s = mk<C>((T)1, (T)0);
+            bool has_s = false;
+            if (a.eoA) {
+                s = reinterpret_cast<const C *>(a.eoA)[lic / a.rest1];
+                has_s = true;
+            }
+            if (a.eoB) {
+                const C sb = reinterpret_cast<const C *>(a.eoB)[lic % a.rest1];
+                s = has_s ? cmul(s, sb) : sb;
+                has_s = true;
+            }
+            if (a.vrep == VREP_TABLE) {
+                const C *vt = reinterpret_cast<const C *>(a.vtab) + vbase;
+                C h[8];
+#pragma unroll
+                for (int half = 0; half < 2; ++half) {
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) h[q] = ld_table(vt + (half * 8 + q) * U, pol);
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) {
+                        C f = h[q];
+                        if (a.eline) f = cmul(f, reinterpret_cast<const C *>(a.eline)[(half * 8 + q) * U + u]);
+                        if (has_s) f = cmul(f, s);
+                        x[half * 8 + q] = cmul(x[half * 8 + q], f);
+                    }
+                }
+            } else {
+                const double *vt = reinterpret_cast<const double *>(a.vtab) + vbase;
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    C f = expi<T>(ld_table(vt + q * U, pol));
+                    if (a.eline) f = cmul(f, reinterpret_cast<const C *>(a.eline)[q * U + u]);
+                    if (has_s) f = cmul(f, s);
+                    x[q] = cmul(x[q], f);
+                }
+            }
+        };
+
+        mbar_wait(&full[b], (unsigned)((k / NB) & 1));
+        C x[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) x[q] = dense[q * U];
+
+        if constexpr (MODE == MODE_OPEN) phase(x);
+        DifChain<T, N, 0, SIGN>::run(x, u, stw, sl, gb);
+        if constexpr (MODE == MODE_MID) {
+            phase(x);
+            DitChain<T, N, LAST, -SIGN>::run(x, u, stw, sl, gb);
+        } else {
+            // registers hold frequency revB[u] + U q at network position 16 u + q: scatter to natural order
+            C *wa = sl + padp(a.revB[u]);
+            const C *rb = sl + padp(u);
+            gsync(gb);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) wa[lin_delta(q, U)] = x[q];
+            gsync(gb);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) x[q] = rb[lin_delta(q, U)];
+            if constexpr (MODE == MODE_CLOSE) phase(x);
+        }
+
+        gsync(gb);  // every thread of the group is done with the exchange layout
+#pragma unroll
+        for (int q = 0; q < 16; ++q) dense[q * U] = x[q];
+        fence_async_smem();
+        gsync(gb);
+        if (tid == 0) {
+            bulk_store(gpsi + tile * TL * N, buf, tile_bytes);
+            if (k + NB < nloc) {
+                bulk_wait_read();  // the buffer has been read out: refill it with the tile NB ahead
+                issue(k + NB);
+            }
+        }
+    }
+    if (tid == 0) bulk_wait_all();
+}
+
+template <typename T, int N, int MODE, int SIGN, int MAXT>
+cudaError_t launch_ring(const RingArgs &a, unsigned threads, size_t smem, unsigned grid, cudaStream_t st);
+
+}  // namespace sso
