@@ -9,6 +9,7 @@
 //   2D: 2 passes   [F_1^-1 V F_1]  [F_0 K F_0^-1]
 //   3D: 4 passes   [F_2^-1 V F_2]  [F_1]  [F_0 K F_0^-1]  [F_1^-1]
 // plus one opening [F_last V/2] and one closing [V/2 F_last^-1] pass per sso_step call.
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
@@ -179,6 +180,17 @@ static LaunchFn find_launch(int precision, int N, int strided, int pw, int sign)
     return nullptr;
 }
 
+static SRingLaunchFn find_sring(int precision, int N, int mode) {
+    switch (N) {
+#define SSO_CASE(NN) \
+    case NN:         \
+        return precision == SSO_C64 ? sso_sring_lookup_f32_##NN(mode) : sso_sring_lookup_f64_##NN(mode);
+        SSO_FOR_EACH_N(SSO_CASE)
+#undef SSO_CASE
+    }
+    return nullptr;
+}
+
 static RingLaunchFn find_ring(int precision, int N, int mode, int maxt) {
     switch (N) {
 #define SSO_CASE(NN) \
@@ -265,9 +277,12 @@ struct sso_plan {
     void *d_erow[3] = {nullptr, nullptr, nullptr};  // field phase rows of the current call (build_erows_kernel)
     size_t erow_cap[3] = {0, 0, 0};
     bool e_axis_on[3] = {false, false, false};
+    CUtensorMap tmap[3];             // strided-axis tile maps (sso_sring.cuh), valid for tmap_psi / tmap_tl
+    const void *tmap_psi[3] = {nullptr, nullptr, nullptr};
+    int tmap_tl[3] = {0, 0, 0};
     int vrep = VREP_TABLE;
     bool kph_valid = false;
-    int opt_tl_contig = 0, opt_tl_strided = 0, opt_groups = 0, opt_ring = 0, opt_maxt = 0;
+    int opt_tl_contig = 0, opt_tl_strided = 0, opt_groups = 0, opt_ring = 0, opt_maxt = 0, opt_sring = 0;
     int dbg_skip = 0;  // development only: bit 0 skip DIF, bit 1 skip DIT, bit 2 skip the pointwise factor (wrong results)
     double *d_partial = nullptr, *d_norm = nullptr;
     unsigned *d_sched = nullptr;  // tile scheduler of the pass kernel (zero between launches)
@@ -297,6 +312,15 @@ template <typename V> static cudaError_t upload(void **dst, const std::vector<V>
     cudaError_t e = cudaMalloc(dst, src.size() * sizeof(V));
     if (e != cudaSuccess) return e;
     return cudaMemcpy(*dst, src.data(), src.size() * sizeof(V), cudaMemcpyHostToDevice);
+}
+
+// development aid: SSO_DEBUG_SYNC=1 synchronises after every pass and names the one that failed
+static int dbg_sync(sso_plan *plan, cudaStream_t st, const char *what, cudaError_t e) {
+    static int on = -1;
+    if (on < 0) on = getenv("SSO_DEBUG_SYNC") ? 1 : 0;
+    if (e == cudaSuccess && on) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(plan, e, what);
+    return SSO_OK;
 }
 
 static bool is_pow2(long long v) { return v > 0 && (v & (v - 1)) == 0; }
@@ -626,6 +650,10 @@ int sso_set_option(sso_plan *plan, int option, int64_t value) {
             if (value != 0 && value != 384 && value != 512) return fail(plan, SSO_ERR_INVALID, "threads per CTA must be 0, 384 or 512");
             plan->opt_maxt = (int)value;
             return SSO_OK;
+        case SSO_OPT_STRIDED_RING:
+            if (value < 0 || value > 4) return fail(plan, SSO_ERR_INVALID, "strided ring mode must be 0 (auto), 1 (force) or 2 (off)");
+            plan->opt_sring = (int)value;
+            return SSO_OK;
         case SSO_OPT_GROUPS_PER_CTA:
             if (value < 0 || value > 15) return fail(plan, SSO_ERR_INVALID, "groups per CTA must be in [0, 15]");
             plan->opt_groups = (int)value;
@@ -692,7 +720,8 @@ int choose_tl(const sso_plan *p, const Geometry &g, int cc) {
         if (tl < 1) tl = 1;
         if (tl > g.lines) tl = g.lines;
     } else {
-        const int tlmin = 32 / esz < 1 ? 1 : 32 / esz;  // at least one 32-byte sector per line element
+        int tlmin = 64 / esz;  // 64-byte rows: narrower rows are served at less than half speed
+        while (tlmin > 1 && cc * tlmin * U > 512) tlmin /= 2;
         tl = p->opt_tl_strided > 0 ? p->opt_tl_strided : 256 / (cc * U);
         if (p->opt_tl_strided == 0 && tl < tlmin) tl = tlmin;
         if (tl > g.inner) tl = g.inner;
@@ -815,14 +844,42 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
     size_t smem = twbytes + (size_t)G * greg;
     if ((plan->dbg_skip >> 8) & 1) smem = smem < 120 * 1024 ? 120 * 1024 : smem;  // development: one CTA per SM
     cudaError_t e = fn(a, threads, smem, st);
-    if (e != cudaSuccess) return cuda_fail(plan, e, "pass kernel launch");
-    return SSO_OK;
+    return dbg_sync(plan, st, g.strided ? "direct strided pass" : "direct contiguous pass", e);
 }
 
+
+// groups per CTA and buffers per group of a ring pass: GT threads per group, room for bmax buffers,
+// tiles_per_cta tiles to share
+void choose_groups(const sso_plan *plan, int GT, int bmax, long long tiles_per_cta, int *G, int *NBG) {
+    int g = 1, nbg = bmax >= 2 ? 2 : 1;
+    if (GT % 32 == 0) {
+        const int gthr = 512 / GT > 15 ? 15 : 512 / GT;
+        const int g2 = gthr < bmax / 2 ? gthr : bmax / 2;  // double-buffered groups
+        const int g1 = gthr < bmax ? gthr : bmax;          // single-buffered groups
+        if (g2 >= 3 || g2 >= g1) {
+            g = g2;
+            nbg = 2;
+        } else {
+            g = g1;
+            nbg = 1;
+        }
+        if (plan->opt_ring > 0) nbg = plan->opt_ring;
+        if (plan->opt_groups > 0) g = plan->opt_groups;
+        while (g > 1 && (g * GT > 512 || g * nbg > bmax)) --g;
+        while (nbg > 1 && g * nbg > bmax) --nbg;
+        if (g > tiles_per_cta) g = (int)(tiles_per_cta > 0 ? tiles_per_cta : 1);
+        if (g < 1) g = 1;
+    }
+    while (nbg > 1 && nbg * g > bmax) --nbg;
+    if (nbg > 4) nbg = 4;
+    *G = g;
+    *NBG = nbg;
+}
 
 // contiguous-axis pass of a 2D/3D lattice through the ring pipeline (sso_ring.cuh).  `row` selects the field
 // phase row of this call (build_erows_kernel): 0 opening, j merged after step j-1, nsteps closing.
 int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStream_t st) {
+    if (plan->dbg_skip & 32) return SSO_OK;  // development: no potential pass
     const int last = plan->ndim - 1;
     const Axis &A = plan->ax[last];
     const int U = A.n / 16;
@@ -838,23 +895,14 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     const size_t twbytes = (size_t)twiddle_count_padded(A.n) * esz;
     const long long ntiles = lines * plan->ncomp / TL;
     if (ntiles > 0x7fffffffLL) return fail(plan, SSO_ERR_UNSUPPORTED, "too many tiles");
-    const int maxt = plan->opt_maxt == 384 ? 384 : 512;
-    int G = 1;
-    if (GT % 32 == 0) {
-        G = plan->opt_groups > 0 ? plan->opt_groups : maxt / GT;
-        while (G > 1 && G * GT > maxt) --G;
-        if (G > 15) G = 15;
-        const long long per_sm = (ntiles + 147) / 148;
-        if (G > per_sm) G = (int)per_sm;
-        if (G < 1) G = 1;
-    }
+    // G groups, each with its own NBG buffers (NBG = 2: the next tile loads while the current one is worked on)
     const size_t avail = 227 * 1024 - 256 - twbytes;
-    int NB = (int)(avail / bufbytes);
-    const int want = plan->opt_ring > 0 ? plan->opt_ring : G + 2 + G / 2;
-    if (NB > want) NB = want;
-    if (NB > 16) NB = 16;
-    if (NB < 1) return fail(plan, SSO_ERR_UNSUPPORTED, "line too long for the ring pipeline");
-    if (G > NB) G = NB;
+    const int bmax = (int)(avail / bufbytes);
+    if (bmax < 1) return fail(plan, SSO_ERR_UNSUPPORTED, "line too long for the ring pipeline");
+    int G = 1, NBG = 1;
+    choose_groups(plan, GT, bmax, (ntiles + 147) / 148, &G, &NBG);
+    const int maxt = plan->opt_maxt ? plan->opt_maxt : (G * GT <= 384 ? 384 : 512);
+    const int NB = G * NBG;
     RingArgs a{};
     a.psi = psi;
     a.tw = A.tw;
@@ -881,8 +929,122 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     const size_t smem = twbytes + (size_t)NB * bufbytes + (size_t)NB * 8;
     const unsigned grid = (unsigned)(ntiles < 148 ? ntiles : 148);
     cudaError_t e = fn(a, (unsigned)(G * GT), smem, grid, st);
-    if (e != cudaSuccess) return cuda_fail(plan, e, "ring kernel launch");
-    return SSO_OK;
+    return dbg_sync(plan, st, mode == MODE_OPEN ? "ring opening pass" : (mode == MODE_MID ? "ring potential pass" : "ring closing pass"), e);
+}
+
+
+// ---- strided-axis passes through the TMA ring (sso_sring.cuh) -------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                  const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+struct SRingShape {
+    bool ok;
+    int TL, GT, G, NB, pitch, box_rows;
+    size_t bufbytes, twbytes;
+};
+
+// tile shape of a strided pass, or ok = false when the ring does not fit (the direct kernel takes over)
+SRingShape sring_shape(const sso_plan *plan, int axis, int cc) {
+    SRingShape r{};
+    if (plan->opt_sring == 2 || !encode_tiled_fn()) return r;
+    const Axis &A = plan->ax[axis];
+    const Geometry g = geometry(plan, axis);
+    const int U = A.n / 16, esz = (int)plan->esize();
+    int TL = plan->opt_tl_strided > 0 ? plan->opt_tl_strided : 128 / esz;  // 128-byte rows
+    const int tlmin = 64 / esz;
+    while (TL > tlmin && (cc * TL * U > 512 || TL > g.inner)) TL /= 2;
+    if (TL < tlmin || TL > g.inner || cc * TL * U > 512 || g.inner % TL != 0) return r;
+    r.TL = TL;
+    r.GT = cc * TL * U;
+    if (r.GT % 32 != 0) return r;
+    const int Gn = 128 / esz;
+    r.pitch = A.n + A.n / 16 + (Gn / TL > 1 ? Gn / TL : 1);
+    r.bufbytes = ((size_t)cc * TL * r.pitch * esz + 127) & ~(size_t)127;
+    r.twbytes = (size_t)twiddle_count_padded(A.n) * esz;
+    const int bmax = (int)((227 * 1024 - 256 - r.twbytes) / r.bufbytes);
+    if (bmax < 1) return r;
+    int NBG = 1;
+    const long long outer = plan->npts / (A.n * g.inner);
+    const long long ntiles = (cc == 1 ? outer * plan->ncomp : 1) * (g.inner / TL);
+    choose_groups(plan, r.GT, bmax, (ntiles + 147) / 148, &r.G, &NBG);
+    if (r.G * NBG < 2 && plan->opt_sring != 1) return r;  // a ring that cannot overlap is no better than the direct kernel
+    r.NB = r.G * NBG;
+    r.box_rows = A.n < 256 ? A.n : 256;
+    r.ok = true;
+    return r;
+}
+
+int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long n, const SRingShape &sh, cudaStream_t st) {
+    if ((plan->dbg_skip & 16) && axis == 0) return SSO_OK;  // development: no kinetic pass
+    const Axis &A = plan->ax[axis];
+    const Geometry g = geometry(plan, axis);
+    const int esz = (int)plan->esize();
+    const int cc = smode == SMODE_KD2 ? 2 : (smode == SMODE_KD4 ? 4 : 1);
+    if (plan->tmap_psi[axis] != psi || plan->tmap_tl[axis] != sh.TL) {
+        const long long outer_c = plan->npts / (A.n * g.inner) * plan->ncomp;
+        cuuint64_t gdim[3] = {(cuuint64_t)(2 * g.inner), (cuuint64_t)A.n, (cuuint64_t)outer_c};
+        cuuint64_t gstr[2] = {(cuuint64_t)(g.inner * esz), (cuuint64_t)((long long)A.n * g.inner * esz)};
+        cuuint32_t box[3] = {(cuuint32_t)(2 * sh.TL), (cuuint32_t)sh.box_rows, 1u};
+        cuuint32_t estr[3] = {1u, 1u, 1u};
+        CUresult cr = encode_tiled_fn()(&plan->tmap[axis], plan->precision == SSO_C128 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, psi,
+                                        gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                        sh.TL * esz >= 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
+                                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (cr != CUDA_SUCCESS) return fail(plan, SSO_ERR_CUDA, "cuTensorMapEncodeTiled failed");
+        plan->tmap_psi[axis] = psi;
+        plan->tmap_tl[axis] = sh.TL;
+    }
+    SRingArgs a{};
+    a.tw = A.tw;
+    a.TL = sh.TL;
+    a.pitch = sh.pitch;
+    a.G = sh.G;
+    a.GT = sh.GT;
+    a.NB = sh.NB;
+    a.bufstride = (int)(sh.bufbytes / esz);
+    a.tiles_per_outer = (int)(g.inner / sh.TL);
+    a.box_rows = sh.box_rows;
+    a.rest1 = g.rest1;
+    const long long outer = plan->npts / (A.n * g.inner);
+    const long long ntiles = (cc == 1 ? outer * plan->ncomp : 1) * a.tiles_per_outer;
+    if (ntiles > 0x7fffffffLL) return fail(plan, SSO_ERR_UNSUPPORTED, "too many tiles");
+    a.ntiles = (int)ntiles;
+    a.ndim = plan->ndim;
+    a.mass = plan->mass;
+    a.clight = plan->clight;
+    a.dt = plan->dt;
+    a.scale = 1.0 / (double)plan->npts;
+    if (smode == SMODE_KS) {
+        a.kph0 = A.d_kph;
+        a.kph1 = g.oaxA >= 0 ? plan->ax[g.oaxA].d_kph : nullptr;
+        a.kph2 = g.oaxB >= 0 ? plan->ax[g.oaxB].d_kph : nullptr;
+    } else if (cc > 1) {
+        a.kv0 = A.d_kv;
+        a.kv1 = g.oaxA >= 0 ? plan->ax[g.oaxA].d_kv : nullptr;
+        a.kv2 = g.oaxB >= 0 ? plan->ax[g.oaxB].d_kv : nullptr;
+        if (plan->field_kind == SSO_FIELD_A)
+            for (int ax = 0; ax < plan->ndim; ++ax) a.sh[ax] = plan->charge * plan->h_avg[(size_t)n * plan->ndim + ax];
+    }
+    SRingLaunchFn fn = find_sring(plan->precision, A.n, smode);
+    if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no strided ring kernel built for this line length");
+    const size_t smem = sh.twbytes + (size_t)sh.NB * sh.bufbytes + (size_t)sh.NB * 8;
+    const unsigned grid = (unsigned)(ntiles < 148 ? ntiles : 148);
+    cudaError_t e = fn(a, &plan->tmap[axis], (unsigned)(a.G * sh.GT), smem, grid, st);
+    return dbg_sync(plan, st, smode == SMODE_DIF ? "strided ring DIF pass" : (smode == SMODE_DIT ? "strided ring DIT pass" : "strided ring kinetic pass"), e);
 }
 
 // field phase rows for steps [n0, n0 + ns) of a 2D/3D call
@@ -1002,6 +1164,10 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
     } else {
         // chunks that share one set of field phase rows; each chunk opens and closes with a half step
         const long long chunk = erow_chunk(plan);
+        SRingShape shk = sring_shape(plan, 0, plan->ncomp == 1 ? 1 : plan->ncomp);
+        SRingShape shm = nd == 3 ? sring_shape(plan, 1, 1) : SRingShape{};
+        if (plan->opt_sring == 3) shm.ok = false;  // development: kinetic pass only
+        if (plan->opt_sring == 4) shk.ok = false;  // development: middle-axis passes only
         for (long long c0 = 0; c0 < nsteps; c0 += chunk) {
             const long long ns = nsteps - c0 < chunk ? nsteps - c0 : chunk;
             const long long nb = n0 + c0;
@@ -1011,15 +1177,27 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
             for (long long s = 0; s < ns; ++s) {
                 const long long n = nb + s;
                 if (plan->ncomp == 1 && (rc = build_kphase(plan, n, st)) != SSO_OK) return rc;
-                if (nd == 3) {
-                    PassSpec mid{1, PW_NONE, -1, 1, 0, 0, 0, 0, 0, 0, 1, n};  // F_1, stored in network order
-                    if ((rc = launch(plan, psi, mid, st)) != SSO_OK) return rc;
+                if (nd == 3) {  // F_1, stored in network order
+                    if (shm.ok) rc = launch_sring_pass(plan, psi, 1, SMODE_DIF, n, shm, st);
+                    else {
+                        PassSpec mid{1, PW_NONE, -1, 1, 0, 0, 0, 0, 0, 0, 1, n};
+                        rc = launch(plan, psi, mid, st);
+                    }
+                    if (rc != SSO_OK) return rc;
                 }
-                PassSpec kin{0, kpw, -1, 1, 1, 0, 1, 0, 0, 0, 1, n};  // F_0 K F_0^-1
-                if ((rc = launch(plan, psi, kin, st)) != SSO_OK) return rc;
-                if (nd == 3) {
-                    PassSpec mid{1, PW_NONE, -1, 0, 1, 0, 0, 0, 0, 0, 1, n};  // F_1^-1 from network order
-                    if ((rc = launch(plan, psi, mid, st)) != SSO_OK) return rc;
+                if (shk.ok) rc = launch_sring_pass(plan, psi, 0, kpw == PW_KS ? SMODE_KS : (kpw == PW_KD2 ? SMODE_KD2 : SMODE_KD4), n, shk, st);
+                else {
+                    PassSpec kin{0, kpw, -1, 1, 1, 0, 1, 0, 0, 0, 1, n};  // F_0 K F_0^-1
+                    rc = launch(plan, psi, kin, st);
+                }
+                if (rc != SSO_OK) return rc;
+                if (nd == 3) {  // F_1^-1 from network order
+                    if (shm.ok) rc = launch_sring_pass(plan, psi, 1, SMODE_DIT, n, shm, st);
+                    else {
+                        PassSpec mid{1, PW_NONE, -1, 0, 1, 0, 0, 0, 0, 0, 1, n};
+                        rc = launch(plan, psi, mid, st);
+                    }
+                    if (rc != SSO_OK) return rc;
                 }
                 // F_last^-1 V(n, n+1) F_last, or the closing F_last^-1, V/2
                 if ((rc = launch_ring_pass(plan, psi, s + 1 < ns ? MODE_MID : MODE_CLOSE, s + 1, st)) != SSO_OK) return rc;

@@ -93,6 +93,31 @@ struct RingArgs {
 };
 
 using RingLaunchFn = cudaError_t (*)(const RingArgs &, unsigned threads, size_t smem, unsigned grid, cudaStream_t st);
+
+// strided-axis passes through the same ring, tiles moved as TMA tensor boxes (sso_sring.cuh)
+enum : int { SMODE_KS = 0, SMODE_KD2 = 1, SMODE_KD4 = 2, SMODE_DIF = 3, SMODE_DIT = 4 };
+struct SRingArgs {
+    const void *tw;           // twiddle blocks of the line axis
+    int ntiles;               // tiles of TL adjacent lines (x all components when they are independent)
+    int TL;                   // adjacent lines per tile: one row of a tile is TL complex numbers, contiguous in memory
+    int pitch;                // padded line pitch of the exchange layout (complex elements)
+    int G, GT, NB, bufstride; // as in RingArgs; GT = CC * TL * N/16
+    int tiles_per_outer;      // inner / TL
+    int box_rows;             // rows per TMA box (<= 256); a tile is CC * N / box_rows boxes
+    int rest1;                // line = ia * rest1 + ib on the non-line axes
+    // kinetic factor (step-dependent shifts are resolved on the host)
+    const void *kph0, *kph1, *kph2;  // Schroedinger phase tables (PassArgs)
+    const double *kv0, *kv1, *kv2;   // Dirac k grids (PassArgs)
+    double sh[3];                    // q Abar_n per axis (SSO_FIELD_A), else 0
+    double mass, clight, dt, scale;
+    int ndim;
+};
+using SRingLaunchFn = cudaError_t (*)(const SRingArgs &, const void *tensor_map, unsigned threads, size_t smem, unsigned grid, cudaStream_t st);
+#define SSO_DECL_SRING(N)                            \
+    SRingLaunchFn sso_sring_lookup_f32_##N(int mode); \
+    SRingLaunchFn sso_sring_lookup_f64_##N(int mode);
+SSO_FOR_EACH_N(SSO_DECL_SRING)
+#undef SSO_DECL_SRING
 #define SSO_DECL_RING(N)                                  \
     RingLaunchFn sso_ring_lookup_f32_##N(int mode, int maxt); \
     RingLaunchFn sso_ring_lookup_f64_##N(int mode, int maxt);

@@ -4,6 +4,7 @@
 // dispatcher in sso_api.cu calls.
 #include "sso_pass.cuh"
 #include "sso_ring.cuh"
+#include "sso_sring.cuh"
 #include "sso_dispatch.h"
 
 #ifndef SSO_T
@@ -63,11 +64,40 @@ cudaError_t launch_ring(const RingArgs &a, unsigned threads, size_t smem, unsign
     return cudaGetLastError();
 }
 
+template <typename T, int N, int SMODE>
+cudaError_t launch_sring(const SRingArgs &a, const void *tensor_map, unsigned threads, size_t smem, unsigned grid, cudaStream_t st) {
+    auto kern = sring_kernel<T, N, SMODE>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    if (threads > 512u) return cudaErrorInvalidConfiguration;
+    kern<<<grid, threads, smem, st>>>(a, *reinterpret_cast<const CUtensorMap *>(tensor_map));
+    return cudaGetLastError();
+}
+
 #define SSO_CAT3_(a, b, c) a##b##_##c
 #define SSO_CAT3(a, b, c) SSO_CAT3_(a, b, c)
 
 #define SSO_CAT4_(a, b, c) a##b##_##c
 #define SSO_CAT4(a, b, c) SSO_CAT4_(a, b, c)
+#ifdef SSO_STUB
+SRingLaunchFn SSO_CAT4(sso_sring_lookup_, SSO_TNAME, SSO_N)(int) { return nullptr; }
+#else
+SRingLaunchFn SSO_CAT4(sso_sring_lookup_, SSO_TNAME, SSO_N)(int mode) {
+    using T = SSO_T;
+    constexpr int N = SSO_N;
+    if (mode == SMODE_KS) return &launch_sring<T, N, SMODE_KS>;
+    if (mode == SMODE_KD2) return &launch_sring<T, N, SMODE_KD2>;
+    if (mode == SMODE_KD4) return &launch_sring<T, N, SMODE_KD4>;
+    if (mode == SMODE_DIF) return &launch_sring<T, N, SMODE_DIF>;
+    if (mode == SMODE_DIT) return &launch_sring<T, N, SMODE_DIT>;
+    return nullptr;
+}
+#endif
+
 #ifdef SSO_STUB
 RingLaunchFn SSO_CAT4(sso_ring_lookup_, SSO_TNAME, SSO_N)(int, int) { return nullptr; }
 #else

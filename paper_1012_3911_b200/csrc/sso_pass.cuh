@@ -277,6 +277,74 @@ template <typename T> __device__ __forceinline__ typename CxOf<T>::type expi(dou
     return mk<typename CxOf<T>::type>((T)c, (T)s);
 }
 
+// Dirac kinetic factor on the DIF output (eq. 27-33 in the closed form
+// U = cos(E tau) - i sin(E tau)/E (c alpha.pi + m c^2 beta), see the file header): the CC components of a k point
+// are gathered into one thread through the exchange buffers, multiplied by the 2x2 / 4x4 unitary and scattered
+// back.  line0 = exchange line of (component 0, this thread's t); comp_pitch = elements between components.
+template <typename T, int CC, int U>
+__device__ __forceinline__ void dirac_kinetic(typename CxOf<T>::type (&x)[16], int u, int c, typename CxOf<T>::type *sl, typename CxOf<T>::type *line0,
+                                              int comp_pitch, int gb, const double *__restrict__ kv0, double sh0, double p1, double p2, double mass,
+                                              double clight, double dt, double scale) {
+    using C = typename CxOf<T>::type;
+    constexpr int PP = 16 / CC;
+    // all components of a k point into one thread: thread (c, u) takes the PP points
+    // 16 u + c PP + i of every component
+    C *me = sl + 17 * u;
+    gsync(gb);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) me[q] = x[q];
+    gsync(gb);
+    C y[CC][PP];
+#pragma unroll
+    for (int c2 = 0; c2 < CC; ++c2)
+#pragma unroll
+        for (int i = 0; i < PP; ++i) y[c2][i] = line0[c2 * comp_pitch + 17 * u + c * PP + i];
+    const double mc2 = mass * clight * clight;
+#pragma unroll
+    for (int i = 0; i < PP; ++i) {
+        const int q2 = c * PP + i;
+        const double p0 = kv0[q2 * U + u] - sh0;
+        const double pp = p0 * p0 + p1 * p1 + p2 * p2;
+        const double E = sqrt(clight * clight * pp + mc2 * mc2);
+        double sn, cs;
+        sincos(E * dt, &sn, &cs);
+        double sE = E > 0.0 ? sn / E : dt;
+        cs *= scale;
+        sE *= scale;
+        const T fc = (T)cs;
+        const T fm = (T)(sE * mc2);
+        const T f0 = (T)(sE * clight * p0), f1 = (T)(sE * clight * p1), f2 = (T)(sE * clight * p2);
+        // out = cs psi - i sE H psi ;  (-i)(a + i b) = b - i a
+        if constexpr (CC == 2) {
+            const C a0 = y[0][i], a1 = y[1][i];
+            // H psi_0 = mc2 a0 + c (p0 - i p1) a1 ; H psi_1 = c (p0 + i p1) a0 - mc2 a1
+            const C h0 = mk<C>(fm * a0.x + f0 * a1.x + f1 * a1.y, fm * a0.y + f0 * a1.y - f1 * a1.x);
+            const C h1 = mk<C>(f0 * a0.x - f1 * a0.y - fm * a1.x, f0 * a0.y + f1 * a0.x - fm * a1.y);
+            y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
+            y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
+        } else {
+            const C a0 = y[0][i], a1 = y[1][i], a2 = y[2][i], a3 = y[3][i];
+            // sigma.p (v0, v1) = (p2 v0 + (p0 - i p1) v1, (p0 + i p1) v0 - p2 v1)
+            // H psi = (mc2 u + c sigma.p l, c sigma.p u - mc2 l)
+            const C h0 = mk<C>(fm * a0.x + f2 * a2.x + f0 * a3.x + f1 * a3.y, fm * a0.y + f2 * a2.y + f0 * a3.y - f1 * a3.x);
+            const C h1 = mk<C>(fm * a1.x + f0 * a2.x - f1 * a2.y - f2 * a3.x, fm * a1.y + f0 * a2.y + f1 * a2.x - f2 * a3.y);
+            const C h2 = mk<C>(f2 * a0.x + f0 * a1.x + f1 * a1.y - fm * a2.x, f2 * a0.y + f0 * a1.y - f1 * a1.x - fm * a2.y);
+            const C h3 = mk<C>(f0 * a0.x - f1 * a0.y - f2 * a1.x - fm * a3.x, f0 * a0.y + f1 * a0.x - f2 * a1.y - fm * a3.y);
+            y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
+            y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
+            y[2][i] = mk<C>(fc * a2.x + h2.y, fc * a2.y - h2.x);
+            y[3][i] = mk<C>(fc * a3.x + h3.y, fc * a3.y - h3.x);
+        }
+    }
+#pragma unroll
+    for (int c2 = 0; c2 < CC; ++c2)
+#pragma unroll
+        for (int i = 0; i < PP; ++i) line0[c2 * comp_pitch + 17 * u + c * PP + i] = y[c2][i];
+    gsync(gb);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) x[q] = me[q];
+}
+
 // step average row n, component ax (0 when there is no table)
 __device__ __forceinline__ double favg(const PassArgs &a, long long n, int ax) {
     return a.step_avg ? a.step_avg[n * a.ndim + ax] : 0.0;
@@ -523,62 +591,7 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
                         p1 = a.kv1[ia] - sh[1];
                         p2 = a.kv2[ib] - sh[2];
                     }
-                    // all components of a k point into one thread: thread (c, u) takes the PP points
-                    // 16 u + c PP + i of every component
-                    C *me = sl + 17 * u;
-                    gsync(gb);
-#pragma unroll
-                    for (int q = 0; q < 16; ++q) me[q] = x[q];
-                    gsync(gb);
-                    C y[CC][PP];
-#pragma unroll
-                    for (int c2 = 0; c2 < CC; ++c2)
-#pragma unroll
-                        for (int i = 0; i < PP; ++i) y[c2][i] = smg[(c2 * TL + t) * a.pitch + 17 * u + c * PP + i];
-                    const double mc2 = a.mass * a.clight * a.clight;
-#pragma unroll
-                    for (int i = 0; i < PP; ++i) {
-                        const int q2 = c * PP + i;
-                        const double p0 = a.kv0[q2 * U + u] - sh[0];
-                        const double pp = p0 * p0 + p1 * p1 + p2 * p2;
-                        const double E = sqrt(a.clight * a.clight * pp + mc2 * mc2);
-                        double sn, cs;
-                        sincos(E * a.dt, &sn, &cs);
-                        double sE = E > 0.0 ? sn / E : a.dt;
-                        cs *= a.scale;
-                        sE *= a.scale;
-                        const T fc = (T)cs;
-                        const T fm = (T)(sE * mc2);
-                        const T f0 = (T)(sE * a.clight * p0), f1 = (T)(sE * a.clight * p1), f2 = (T)(sE * a.clight * p2);
-                        // out = cs psi - i sE H psi ;  (-i)(a + i b) = b - i a
-                        if constexpr (CC == 2) {
-                            const C a0 = y[0][i], a1 = y[1][i];
-                            // H psi_0 = mc2 a0 + c (p0 - i p1) a1 ; H psi_1 = c (p0 + i p1) a0 - mc2 a1
-                            const C h0 = mk<C>(fm * a0.x + f0 * a1.x + f1 * a1.y, fm * a0.y + f0 * a1.y - f1 * a1.x);
-                            const C h1 = mk<C>(f0 * a0.x - f1 * a0.y - fm * a1.x, f0 * a0.y + f1 * a0.x - fm * a1.y);
-                            y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
-                            y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
-                        } else {
-                            const C a0 = y[0][i], a1 = y[1][i], a2 = y[2][i], a3 = y[3][i];
-                            // sigma.p (v0, v1) = (p2 v0 + (p0 - i p1) v1, (p0 + i p1) v0 - p2 v1)
-                            // H psi = (mc2 u + c sigma.p l, c sigma.p u - mc2 l)
-                            const C h0 = mk<C>(fm * a0.x + f2 * a2.x + f0 * a3.x + f1 * a3.y, fm * a0.y + f2 * a2.y + f0 * a3.y - f1 * a3.x);
-                            const C h1 = mk<C>(fm * a1.x + f0 * a2.x - f1 * a2.y - f2 * a3.x, fm * a1.y + f0 * a2.y + f1 * a2.x - f2 * a3.y);
-                            const C h2 = mk<C>(f2 * a0.x + f0 * a1.x + f1 * a1.y - fm * a2.x, f2 * a0.y + f0 * a1.y - f1 * a1.x - fm * a2.y);
-                            const C h3 = mk<C>(f0 * a0.x - f1 * a0.y - f2 * a1.x - fm * a3.x, f0 * a0.y + f1 * a0.x - f2 * a1.y - fm * a3.y);
-                            y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
-                            y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
-                            y[2][i] = mk<C>(fc * a2.x + h2.y, fc * a2.y - h2.x);
-                            y[3][i] = mk<C>(fc * a3.x + h3.y, fc * a3.y - h3.x);
-                        }
-                    }
-#pragma unroll
-                    for (int c2 = 0; c2 < CC; ++c2)
-#pragma unroll
-                        for (int i = 0; i < PP; ++i) smg[(c2 * TL + t) * a.pitch + 17 * u + c * PP + i] = y[c2][i];
-                    gsync(gb);
-#pragma unroll
-                    for (int q = 0; q < 16; ++q) x[q] = me[q];
+                    dirac_kinetic<T, CC, U>(x, u, c, sl, smg + t * a.pitch, TL * a.pitch, gb, a.kv0, sh[0], p1, p2, a.mass, a.clight, a.dt, a.scale);
                 }
             }
 

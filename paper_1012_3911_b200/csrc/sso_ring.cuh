@@ -103,8 +103,7 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     C *gpsi = reinterpret_cast<C *>(a.psi);
 
     // issue the load of local tile k into its ring buffer, and ask L2 for that tile's potential-phase lines
-    auto issue = [&](int k) {
-        const int b = k % NB;
+    auto issue = [&](int k, int b) {
         const long long tile = (long long)blockIdx.x + (long long)k * gridDim.x;
         mbar_expect_tx(&full[b], tile_bytes);
         bulk_load(bufs + (size_t)b * a.bufstride, gpsi + tile * TL * N, tile_bytes, &full[b]);
@@ -123,11 +122,14 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
         for (int i = threadIdx.x; i < TWN; i += blockDim.x) stw[i] = gtw[i];
     }
     __syncthreads();
-    if (threadIdx.x == 0)
-        for (int k = 0; k < NB && k < nloc; ++k) issue(k);
+    // every group owns NBG = NB / G buffers: its leader fills them, its threads consume them, so a buffer's
+    // mbarrier never sees a waiter that is not in step with its fills
+    const int NBG = NB / G;
+    if (tid == 0)
+        for (int j = 0; j < NBG && grp + j * G < nloc; ++j) issue(grp + j * G, grp * NBG + j);
 
-    for (int k = grp; k < nloc; k += G) {
-        const int b = k % NB;
+    for (int k = grp, j = 0; k < nloc; k += G, ++j) {
+        const int b = grp * NBG + j % NBG;
         C *buf = bufs + (size_t)b * a.bufstride;
         C *dense = buf + t * N + u;          // bulk-copy layout: [TL][N]
         C *sl = buf + t * a.pitch;           // exchange layout: padded lines
@@ -175,7 +177,7 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
             }
         };
 
-        mbar_wait(&full[b], (unsigned)((k / NB) & 1));
+        mbar_wait(&full[b], (unsigned)((j / NBG) & 1));
         C x[16];
 #pragma unroll
         for (int q = 0; q < 16; ++q) x[q] = dense[q * U];
@@ -205,9 +207,9 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
         gsync(gb);
         if (tid == 0) {
             bulk_store(gpsi + tile * TL * N, buf, tile_bytes);
-            if (k + NB < nloc) {
-                bulk_wait_read();  // the buffer has been read out: refill it with the tile NB ahead
-                issue(k + NB);
+            if (k + NBG * G < nloc) {
+                bulk_wait_read();  // the buffer has been read out: refill it with this group's tile NBG ahead
+                issue(k + NBG * G, b);
             }
         }
     }
