@@ -853,7 +853,8 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
 void choose_groups(const sso_plan *plan, int GT, int bmax, long long tiles_per_cta, int *G, int *NBG) {
     int g = 1, nbg = bmax >= 2 ? 2 : 1;
     if (GT % 32 == 0) {
-        const int gthr = 512 / GT > 15 ? 15 : 512 / GT;
+        const int cap = plan->opt_maxt ? plan->opt_maxt : 512;
+        const int gthr = cap / GT > 15 ? 15 : cap / GT;
         const int g2 = gthr < bmax / 2 ? gthr : bmax / 2;  // double-buffered groups
         const int g1 = gthr < bmax ? gthr : bmax;          // single-buffered groups
         if (g2 >= 3 || g2 >= g1) {
@@ -865,7 +866,7 @@ void choose_groups(const sso_plan *plan, int GT, int bmax, long long tiles_per_c
         }
         if (plan->opt_ring > 0) nbg = plan->opt_ring;
         if (plan->opt_groups > 0) g = plan->opt_groups;
-        while (g > 1 && (g * GT > 512 || g * nbg > bmax)) --g;
+        while (g > 1 && (g * GT > cap || g * nbg > bmax)) --g;
         while (nbg > 1 && g * nbg > bmax) --nbg;
         if (g > tiles_per_cta) g = (int)(tiles_per_cta > 0 ? tiles_per_cta : 1);
         if (g < 1) g = 1;
@@ -964,14 +965,30 @@ SRingShape sring_shape(const sso_plan *plan, int axis, int cc) {
     const Axis &A = plan->ax[axis];
     const Geometry g = geometry(plan, axis);
     const int U = A.n / 16, esz = (int)plan->esize();
-    int TL = plan->opt_tl_strided > 0 ? plan->opt_tl_strided : 128 / esz;  // 128-byte rows
-    const int tlmin = 64 / esz;
-    while (TL > tlmin && (cc * TL * U > 512 || TL > g.inner)) TL /= 2;
-    if (TL < tlmin || TL > g.inner || cc * TL * U > 512 || g.inner % TL != 0) return r;
+    // rows of 128 bytes when two or more buffers of such tiles fit; else narrower rows (TMA serves 32-byte rows
+    // better than per-thread loads do), down to one buffer holding the widest tile that fits
+    const int Gn = 128 / esz;
+    auto fits = [&](int TL, int *bmax_out) {
+        if (TL < 1 || TL > g.inner || g.inner % TL != 0 || cc * TL * U > 512 || (cc * TL * U) % 32 != 0) return false;
+        const int pitch = A.n + A.n / 16 + (Gn / TL > 1 ? Gn / TL : 1);
+        const size_t bb = ((size_t)cc * TL * pitch * esz + 127) & ~(size_t)127;
+        const size_t tw = (size_t)twiddle_count_padded(A.n) * esz;
+        if (bb + tw > 227 * 1024 - 256) return false;
+        *bmax_out = (int)((227 * 1024 - 256 - tw) / bb);
+        return true;
+    };
+    int TL = 0, bm = 0;
+    if (plan->opt_tl_strided > 0) {
+        if (fits(plan->opt_tl_strided, &bm)) TL = plan->opt_tl_strided;
+    } else {
+        for (int cand = 128 / esz; cand >= 32 / esz && cand >= 1 && !TL; cand /= 2)
+            if (fits(cand, &bm) && bm >= 2) TL = cand;
+        for (int cand = 128 / esz; cand >= 32 / esz && cand >= 1 && !TL; cand /= 2)
+            if (fits(cand, &bm)) TL = cand;
+    }
+    if (!TL) return r;
     r.TL = TL;
     r.GT = cc * TL * U;
-    if (r.GT % 32 != 0) return r;
-    const int Gn = 128 / esz;
     r.pitch = A.n + A.n / 16 + (Gn / TL > 1 ? Gn / TL : 1);
     r.bufbytes = ((size_t)cc * TL * r.pitch * esz + 127) & ~(size_t)127;
     r.twbytes = (size_t)twiddle_count_padded(A.n) * esz;
@@ -981,7 +998,6 @@ SRingShape sring_shape(const sso_plan *plan, int axis, int cc) {
     const long long outer = plan->npts / (A.n * g.inner);
     const long long ntiles = (cc == 1 ? outer * plan->ncomp : 1) * (g.inner / TL);
     choose_groups(plan, r.GT, bmax, (ntiles + 147) / 148, &r.G, &NBG);
-    if (r.G * NBG < 2 && plan->opt_sring != 1) return r;  // a ring that cannot overlap is no better than the direct kernel
     r.NB = r.G * NBG;
     r.box_rows = A.n < 256 ? A.n : 256;
     r.ok = true;

@@ -85,6 +85,7 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     constexpr int LAST = Sched<N>::M - 1;
     constexpr int TWN = Sched<N>::twoff(LAST);
     constexpr int TWP = (TWN + 7) & ~7;
+    constexpr bool EARLY = MODE == MODE_MID && (sizeof(T) == 4 || MAXT == 384);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     C *stw = reinterpret_cast<C *>(smem_raw);
     C *bufs = stw + TWP;
@@ -138,6 +139,16 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
         const size_t vbase = (size_t)lic * N + u;
 
         // pointwise factor of this pass for register q (table slot q U + u of line lic)
+        // with registers to spare (complex64, or the 384-thread build) the merged-phase line is requested before
+        // the tile is even waited for, so that its latency hides behind the first transform
+        [[maybe_unused]] C hh[EARLY ? 16 : 1];
+        if constexpr (EARLY) {
+            if (a.vrep == VREP_TABLE) {
+                const C *vt = reinterpret_cast<const C *>(a.vtab) + vbase;
+#pragma unroll
+                for (int q = 0; q < 16; ++q) hh[q] = ld_table(vt + q * U, pol);
+            }
+        }
         auto phase = [&](C (&x)[16]) {
             C s = mk<C>((T)1, (T)0);
             bool has_s = false;
@@ -152,17 +163,27 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
             }
             if (a.vrep == VREP_TABLE) {
                 const C *vt = reinterpret_cast<const C *>(a.vtab) + vbase;
-                C h[8];
+                if constexpr (EARLY) {
 #pragma unroll
-                for (int half = 0; half < 2; ++half) {
-#pragma unroll
-                    for (int q = 0; q < 8; ++q) h[q] = ld_table(vt + (half * 8 + q) * U, pol);
-#pragma unroll
-                    for (int q = 0; q < 8; ++q) {
-                        C f = h[q];
-                        if (a.eline) f = cmul(f, reinterpret_cast<const C *>(a.eline)[(half * 8 + q) * U + u]);
+                    for (int q = 0; q < 16; ++q) {
+                        C f = hh[q];
+                        if (a.eline) f = cmul(f, reinterpret_cast<const C *>(a.eline)[q * U + u]);
                         if (has_s) f = cmul(f, s);
-                        x[half * 8 + q] = cmul(x[half * 8 + q], f);
+                        x[q] = cmul(x[q], f);
+                    }
+                } else {
+                    C h[8];
+#pragma unroll
+                    for (int half = 0; half < 2; ++half) {
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) h[q] = ld_table(vt + (half * 8 + q) * U, pol);
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) {
+                            C f = h[q];
+                            if (a.eline) f = cmul(f, reinterpret_cast<const C *>(a.eline)[(half * 8 + q) * U + u]);
+                            if (has_s) f = cmul(f, s);
+                            x[half * 8 + q] = cmul(x[half * 8 + q], f);
+                        }
                     }
                 }
             } else {
