@@ -71,7 +71,7 @@ extern "C" {
                                             1 = real angle table + in-kernel sincos polynomial   */
 
 #define SSO_OPT_GROUPS_PER_CTA 4         /* independent line groups per CTA (0 = auto)              */
-#define SSO_OPT_RING_BUFFERS 5           /* tile buffers of the contiguous-axis ring pipeline (0=auto) */
+#define SSO_OPT_RING_BUFFERS 5           /* ring buffers PER GROUP of the ring pipelines (0 = auto: 2 if they fit) */
 #define SSO_OPT_STRIDED_RING 7           /* strided-axis passes: 0 auto, 1 force the TMA ring, 2 direct kernel only */
 #define SSO_OPT_THREADS_PER_CTA 6        /* ring pipeline CTA size: 512 (128 regs/thread) or 384 (168); 0 = auto */
 

@@ -175,3 +175,54 @@ def test_schroedinger_with_vector_potential(torch):
                         step_avg=rng.uniform(-2, 2, size=(4, nd)))
         got, _ = gpu_steps(torch, w, 4)
         assert rel_l2(got, oracle_steps(w, 4)) <= 1e-13
+
+
+# ---------------------------------------------------------------------------------------------------------
+# every pipeline variant computes the same step: direct kernel, forced/disabled TMA ring, group and buffer counts
+# ---------------------------------------------------------------------------------------------------------
+OPT_TL_STRIDED, OPT_GROUPS, OPT_RING, OPT_THREADS, OPT_SRING = 2, 4, 5, 6, 7
+VARIANTS = [
+    ("direct_strided", [(OPT_SRING, 2)]),
+    ("ring_forced", [(OPT_SRING, 1)]),
+    ("ring_rows32B", [(OPT_SRING, 1), (OPT_TL_STRIDED, 2)]),
+    ("one_group", [(OPT_GROUPS, 1)]),
+    ("two_groups_single_buffer", [(OPT_GROUPS, 2), (OPT_RING, 1)]),
+    ("three_buffers", [(OPT_GROUPS, 2), (OPT_RING, 3)]),
+    ("cta384", [(OPT_THREADS, 384)]),
+    ("cta512", [(OPT_THREADS, 512)]),
+]
+
+
+@pytest.mark.parametrize("name,options", VARIANTS, ids=[v[0] for v in VARIANTS])
+def test_pipeline_variants_agree_with_oracle(torch, name, options):
+    cases = [
+        wl.config2(sizes=(256, 256), nsteps=6),        # Schroedinger 2D with E(t)
+        wl.config3(sizes=(64, 128, 64), nsteps=4),     # 3D: middle-axis DIF/DIT passes
+        wl.config4(sizes=(128, 256), nsteps=4),        # Dirac 2 components with A(t)
+        wl.config5(sizes=(64, 32, 64), nsteps=3),      # Dirac 4 components
+    ]
+    for w in cases:
+        n = w.nsteps
+        got, nrm = gpu_steps(torch, w, n, options=options)
+        want = oracle_steps(w, n)
+        assert rel_l2(got, want) <= 1e-13, (name, w.name, rel_l2(got, want))
+        assert abs(nrm - 1.0) < 1e-12
+
+
+def test_many_tiles_per_group_large_lattice(torch):
+    """A lattice large enough that every group of the ring refills its buffers many times (the failure mode of a
+    ring shared between groups showed only beyond 128 MB): F then F^-1 along every axis must return N psi."""
+    sizes = (128, 256, 256)
+    p = sso.Plan(sizes, (0.1, 0.1, 0.1), 0.01, 1, sso.C128)   # V = 0, no field: the step is F^-1 K F
+    g = torch.Generator(device="cuda")
+    g.manual_seed(5)
+    psi0 = torch.randn(sizes, dtype=torch.complex128, device="cuda", generator=g)
+    psi = psi0.clone()
+    p.step(psi, 1)
+    p2 = sso.Plan(sizes, (0.1, 0.1, 0.1), -0.01, 1, sso.C128)
+    p2.step(psi, 1)
+    torch.cuda.synchronize()
+    err = float((psi - psi0).abs().max() / psi0.abs().max())
+    assert err < 1e-13, err
+    p.destroy()
+    p2.destroy()
