@@ -7,7 +7,8 @@ in parallel and links them into paper_1012_3911_b200/libsso.so.  Objects are cac
 paper_1012_3911_b200/build/ and rebuilt when a source or header is newer.
 
 Environment: SSO_SIZES="256,2048" restricts the line lengths that get real kernels (development
-only; the other sizes then report SSO_ERR_UNSUPPORTED), SSO_JOBS sets the parallelism.
+only; the other sizes then report SSO_ERR_UNSUPPORTED), SSO_JOBS sets the parallelism, SSO_NVCC_EXTRA adds
+nvcc flags to the kernel objects (development, e.g. -DSSO_TIMELINE prints a per-phase clock trace of one group).
 """
 from __future__ import annotations
 
@@ -52,6 +53,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     OBJ.mkdir(exist_ok=True)
     sizes_env = os.environ.get("SSO_SIZES")
     real = set(int(s) for s in sizes_env.split(",")) if sizes_env else set(ALL_SIZES)
+    extra = os.environ.get("SSO_NVCC_EXTRA", "").split()  # development: extra nvcc flags (e.g. -DSSO_TIMELINE)
     stamp = _newest_source()
     jobs = []
     objs = []
@@ -65,7 +67,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
             o = OBJ / f"sso_inst_{tname}_{n}{'_stub' if stub else ''}.o"
             objs.append(o)
             if force or not o.exists() or o.stat().st_mtime < stamp:
-                cmd = [nvcc, *NVCC_FLAGS, f"-DSSO_T={t}", f"-DSSO_TNAME={tname}", f"-DSSO_N={n}"]
+                cmd = [nvcc, *NVCC_FLAGS, *extra, f"-DSSO_T={t}", f"-DSSO_TNAME={tname}", f"-DSSO_N={n}"]
                 if stub:
                     cmd.append("-DSSO_STUB")
                 jobs.append(cmd + ["-c", str(CSRC / "sso_inst.cu"), "-o", str(o)])

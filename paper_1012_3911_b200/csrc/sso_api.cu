@@ -916,10 +916,12 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     a.NB = NB;
     a.bufstride = (int)(bufbytes / esz);
     a.lines_per_comp = (int)lines;
+    a.ncomp = plan->ncomp;
     const Geometry g = geometry(plan, last);
     a.rest1 = g.rest1;
     a.vtab = mode == MODE_MID ? plan->d_vfull : plan->d_vtab;
     a.vrep = plan->vrep;
+    a.dbg_nophase = (plan->dbg_skip & 4) ? 1 : 0;
     if (plan->field_kind == SSO_FIELD_E) {
         if (plan->e_axis_on[last]) a.eline = (const char *)plan->d_erow[last] + (size_t)row * A.n * esz;
         if (g.oaxA >= 0 && plan->e_axis_on[g.oaxA]) a.eoA = (const char *)plan->d_erow[g.oaxA] + (size_t)row * plan->ax[g.oaxA].n * esz;
@@ -927,7 +929,7 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     }
     RingLaunchFn fn = find_ring(plan->precision, A.n, mode, maxt);
     if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no ring kernel built for this line length");
-    const size_t smem = twbytes + (size_t)NB * bufbytes + (size_t)NB * 8;
+    const size_t smem = twbytes + (size_t)NB * bufbytes + (size_t)NB * 8 + (size_t)(NB + 1) * 4;
     const unsigned grid = (unsigned)(ntiles < 148 ? ntiles : 148);
     cudaError_t e = fn(a, (unsigned)(G * GT), smem, grid, st);
     return dbg_sync(plan, st, mode == MODE_OPEN ? "ring opening pass" : (mode == MODE_MID ? "ring potential pass" : "ring closing pass"), e);
@@ -1057,7 +1059,7 @@ int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long 
     }
     SRingLaunchFn fn = find_sring(plan->precision, A.n, smode);
     if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no strided ring kernel built for this line length");
-    const size_t smem = sh.twbytes + (size_t)sh.NB * sh.bufbytes + (size_t)sh.NB * 8;
+    const size_t smem = sh.twbytes + (size_t)sh.NB * sh.bufbytes + (size_t)sh.NB * 8 + (size_t)(sh.NB + 1) * 4;
     const unsigned grid = (unsigned)(ntiles < 148 ? ntiles : 148);
     cudaError_t e = fn(a, &plan->tmap[axis], (unsigned)(a.G * sh.GT), smem, grid, st);
     return dbg_sync(plan, st, smode == SMODE_DIF ? "strided ring DIF pass" : (smode == SMODE_DIT ? "strided ring DIT pass" : "strided ring kinetic pass"), e);

@@ -85,11 +85,14 @@ struct RingArgs {
     int NB;                   // ring buffers
     int bufstride;            // complex elements between ring buffers
     int lines_per_comp;       // lines of one component (the potential table repeats per component)
+    int ncomp;                // components; tile index = line block * ncomp + component, so that the tiles that share
+                              // a potential-table block run at the same time and the block is fetched from HBM once
     int rest1;                // table line = ia * rest1 + ib
     const void *vtab;         // MODE_MID: merged phase exp(-i V tau), permuted slots; else exp(-i V tau/2), natural
     int vrep;                 // VREP_TABLE (complex phases) or VREP_ANGLE (real angles, sincos in the kernel)
     const void *eline;        // complex[N] field phase along the line for this pass (same order as vtab) or NULL
     const void *eoA, *eoB;    // complex field phase rows of the other axes, indexed by ia / ib, or NULL
+    int dbg_nophase;          // development only: skip the pointwise factor (wrong results)
 };
 
 using RingLaunchFn = cudaError_t (*)(const RingArgs &, unsigned threads, size_t smem, unsigned grid, cudaStream_t st);

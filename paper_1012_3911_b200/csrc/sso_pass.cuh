@@ -232,19 +232,29 @@ template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void di
 // barrier over one group of a CTA (groups are independent pipelines that share only the twiddle table):
 // gb = 0 means the CTA holds one group (plain __syncthreads), otherwise gb = (named barrier id) | (threads << 8)
 __device__ __forceinline__ void gsync(int gb) {
-    if (gb == 0) __syncthreads();
-    else asm volatile("bar.sync %0, %1;" ::"r"(gb & 15), "r"(gb >> 8) : "memory");
+    if ((gb & 0x3fffffff) == 0) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(gb & 15), "r"((gb & 0x3fffffff) >> 8) : "memory");
 }
+
+// gb flag: consecutive lanes hold consecutive u of one line (contiguous-axis kernels).  The exchange between
+// two stages only moves data inside blocks of max(Mi) consecutive u (Mi = sub-transform length / 16), so when
+// such a block lies inside a warp the group barrier shrinks to a __syncwarp
+constexpr int GB_LANES_ARE_U = 1 << 30;
 
 // registers (layout of stage IA) -> shared memory -> registers (layout of stage IB)
 template <typename T, int N, int IA, int IB> __device__ __forceinline__ void exchange(typename CxOf<T>::type (&x)[16], int u, typename CxOf<T>::type *sl, int gb) {
     using C = typename CxOf<T>::type;
+    constexpr int MiA = Sched<N>::nprev(IA) / 16, MiB = Sched<N>::nprev(IB) / 16;
+    constexpr int SCOPE = MiA > MiB ? MiA : MiB;
     C *wa = sl + stage_base<N, IA>(u);
     const C *rb = sl + stage_base<N, IB>(u);
-    gsync(gb);
+    const bool warp_local = SCOPE <= 32 && (gb & GB_LANES_ARE_U);
+    if (warp_local) __syncwarp();
+    else gsync(gb);
 #pragma unroll
     for (int q = 0; q < 16; ++q) wa[stage_delta<N, IA>(q)] = x[q];
-    gsync(gb);
+    if (warp_local) __syncwarp();
+    else gsync(gb);
 #pragma unroll
     for (int q = 0; q < 16; ++q) x[q] = rb[stage_delta<N, IB>(q)];
 }

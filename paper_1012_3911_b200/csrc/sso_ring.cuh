@@ -15,6 +15,8 @@
 // buffer's store has been read out, NB tiles ahead of its use, and the potential-phase lines of that tile
 // are requested into L2 at the same time.
 #pragma once
+#include <cstdio>
+
 #include "sso_pass.cuh"
 
 namespace sso {
@@ -25,6 +27,9 @@ __device__ __forceinline__ void mbar_init(void *bar, unsigned count) {
 }
 __device__ __forceinline__ void mbar_expect_tx(void *bar, unsigned bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(void *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(void *bar, unsigned parity) {
     asm volatile(
@@ -77,6 +82,26 @@ __device__ __forceinline__ double ld_table(const double *p, uint64_t pol) {
 __device__ __forceinline__ void prefetch_l2_bulk_hint(const void *p, unsigned bytes, uint64_t pol) {
     asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(p), "r"(bytes), "l"(pol) : "memory");
 }
+__device__ __forceinline__ void prefetch_l2_bulk_plain(const void *p, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
+#ifdef SSO_TIMELINE
+#define SSO_TL_DECL long long tl_[12]; int tli_ = 0;
+#define SSO_TL_MARK do { if (tli_ < 12) tl_[tli_++] = clock64(); } while (0)
+#define SSO_TL_DUMP(tag, blk, grp, j)                                                                              \
+    do {                                                                                                           \
+        if (((blk) == 0 || (blk) == 100) && tid == 0 && grp == 1) {                                                       \
+            printf("%s blk %d tile %d (start %lld):", tag, (int)(blk), j, tl_[0] - t_entry_);                                                             \
+            for (int i_ = 1; i_ < tli_; ++i_) printf(" %lld", tl_[i_] - tl_[i_ - 1]);                              \
+            printf("  total %lld\n", tl_[tli_ - 1] - tl_[0]);                                                      \
+        }                                                                                                          \
+    } while (0)
+#else
+#define SSO_TL_DECL
+#define SSO_TL_MARK
+#define SSO_TL_DUMP(tag, blk, grp, j)
+#endif
 
 template <typename T, int N, int MODE, int SIGN, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
@@ -90,11 +115,19 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     C *stw = reinterpret_cast<C *>(smem_raw);
     C *bufs = stw + TWP;
     unsigned long long *full = reinterpret_cast<unsigned long long *>(bufs + (size_t)a.NB * a.bufstride);
+    // ktile[b] = CTA-local tile held by buffer b (-1: none left); ktile[NB] = next unclaimed local tile.  Groups
+    // claim tiles as they finish, so a CTA's tiles are shared evenly even when their count is no multiple of G
+    volatile int *ktile = reinterpret_cast<volatile int *>(full + a.NB);
 
+#ifdef SSO_TIMELINE
+    const long long t_entry_ = clock64();
+#endif
     const int TL = a.TL, GT = a.GT, G = a.G, NB = a.NB;
     const int grp = threadIdx.x / GT;
     const int tid = threadIdx.x - grp * GT;
-    const int gb = G > 1 ? ((grp + 1) | (GT << 8)) : 0;
+    // lanes of a warp hold consecutive u (and whole lines when U < 32): stage exchanges that stay inside 32
+    // consecutive u need no group barrier
+    const int gb = (G > 1 ? ((grp + 1) | (GT << 8)) : 0) | ((U >= 32 || 32 % U == 0) ? GB_LANES_ARE_U : 0);
     const int u = tid % U;
     const int t = tid / U;
     const unsigned tile_bytes = (unsigned)(TL * N * sizeof(C));
@@ -104,17 +137,24 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     C *gpsi = reinterpret_cast<C *>(a.psi);
 
     // issue the load of local tile k into its ring buffer, and ask L2 for that tile's potential-phase lines
+    // tile -> first element of psi and first potential-table line (component fastest)
+    auto tile_elem = [&](long long tile, long long *table_line) {
+        const long long comp = tile % a.ncomp, lb = tile / a.ncomp;
+        *table_line = lb * TL;
+        return (comp * a.lines_per_comp + lb * TL) * (long long)N;
+    };
     auto issue = [&](int k, int b) {
         const long long tile = (long long)blockIdx.x + (long long)k * gridDim.x;
+        long long l0;
+        const long long e0 = tile_elem(tile, &l0);
         mbar_expect_tx(&full[b], tile_bytes);
-        bulk_load(bufs + (size_t)b * a.bufstride, gpsi + tile * TL * N, tile_bytes, &full[b]);
-        if (a.vtab) {
-            const long long l0 = (tile * TL) % a.lines_per_comp;  // a tile never straddles two components
-            prefetch_l2_bulk_hint(reinterpret_cast<const char *>(a.vtab) + (size_t)l0 * N * vesz, (unsigned)(TL * N * vesz), pol);
-        }
+        bulk_load(bufs + (size_t)b * a.bufstride, gpsi + e0, tile_bytes, &full[b]);
+        if (a.vtab && tile % a.ncomp == 0)  // one request per table block
+            prefetch_l2_bulk_plain(reinterpret_cast<const char *>(a.vtab) + (size_t)l0 * N * vesz, (unsigned)(TL * N * vesz));
     };
 
     if (threadIdx.x == 0) {
+        ktile[NB] = NB;
         for (int b = 0; b < NB; ++b) mbar_init(&full[b], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -126,16 +166,31 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     // every group owns NBG = NB / G buffers: its leader fills them, its threads consume them, so a buffer's
     // mbarrier never sees a waiter that is not in step with its fills
     const int NBG = NB / G;
+    // hand a buffer its next tile: load it, or mark the buffer empty and complete its phase by hand
+    auto refill = [&](int kn, int b) {
+        if (kn < nloc) {
+            ktile[b] = kn;
+            issue(kn, b);
+        } else {
+            ktile[b] = -1;
+            mbar_arrive(&full[b]);
+        }
+    };
     if (tid == 0)
-        for (int j = 0; j < NBG && grp + j * G < nloc; ++j) issue(grp + j * G, grp * NBG + j);
+        for (int j = 0; j < NBG; ++j) refill(grp * NBG + j, grp * NBG + j);
 
-    for (int k = grp, j = 0; k < nloc; k += G, ++j) {
+    for (int j = 0;; ++j) {
         const int b = grp * NBG + j % NBG;
+        mbar_wait(&full[b], (unsigned)((j / NBG) & 1));
+        const int k = ktile[b];
+        if (k < 0) break;
         C *buf = bufs + (size_t)b * a.bufstride;
         C *dense = buf + t * N + u;          // bulk-copy layout: [TL][N]
         C *sl = buf + t * a.pitch;           // exchange layout: padded lines
         const long long tile = (long long)blockIdx.x + (long long)k * gridDim.x;
-        const int lic = (int)((tile * TL + t) % a.lines_per_comp);  // line within the component = table line
+        long long l0_;
+        const long long e0_ = tile_elem(tile, &l0_);
+        const int lic = (int)l0_ + t;  // line within the component = table line
         const size_t vbase = (size_t)lic * N + u;
 
         // pointwise factor of this pass for register q (table slot q U + u of line lic)
@@ -198,16 +253,23 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
             }
         };
 
-        mbar_wait(&full[b], (unsigned)((j / NBG) & 1));
+        SSO_TL_DECL
+        SSO_TL_MARK;
+        SSO_TL_MARK;
         C x[16];
 #pragma unroll
         for (int q = 0; q < 16; ++q) x[q] = dense[q * U];
+        gsync(gb);
+        SSO_TL_MARK;  // the exchange layout overlaps the bulk-copy layout of other warps' lines
 
         if constexpr (MODE == MODE_OPEN) phase(x);
         DifChain<T, N, 0, SIGN>::run(x, u, stw, sl, gb);
+        SSO_TL_MARK;
         if constexpr (MODE == MODE_MID) {
-            phase(x);
+            if (!a.dbg_nophase) phase(x);
+            SSO_TL_MARK;
             DitChain<T, N, LAST, -SIGN>::run(x, u, stw, sl, gb);
+            SSO_TL_MARK;
         } else {
             // registers hold frequency revB[u] + U q at network position 16 u + q: scatter to natural order
             C *wa = sl + padp(a.revB[u]);
@@ -221,20 +283,25 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
             if constexpr (MODE == MODE_CLOSE) phase(x);
         }
 
-        gsync(gb);  // every thread of the group is done with the exchange layout
+        gsync(gb);  // every thread of the group is done with the buffer: it can take its next tile right away
+        SSO_TL_MARK;
+        if (tid == 0) refill(atomicAdd(const_cast<int *>(&ktile[NB]), 1), b);
+        // results go straight from registers to global memory (512 contiguous bytes per warp instruction):
+        // no second trip through shared memory and nothing to wait for before the buffer is refilled
+        {
+            C *gout = gpsi + e0_ + (size_t)t * N + u;
 #pragma unroll
-        for (int q = 0; q < 16; ++q) dense[q * U] = x[q];
-        fence_async_smem();
-        gsync(gb);
-        if (tid == 0) {
-            bulk_store(gpsi + tile * TL * N, buf, tile_bytes);
-            if (k + NBG * G < nloc) {
-                bulk_wait_read();  // the buffer has been read out: refill it with this group's tile NBG ahead
-                issue(k + NBG * G, b);
-            }
+            for (int q = 0; q < 16; ++q) st_stream(gout + q * U, x[q]);
         }
+        SSO_TL_MARK;
+        SSO_TL_DUMP("ring", blockIdx.x, grp, j);
     }
-    if (tid == 0) bulk_wait_all();
+#ifdef SSO_TIMELINE
+    const long long t_loop_end_ = clock64();
+#endif
+#ifdef SSO_TIMELINE
+    if ((blockIdx.x == 0 || blockIdx.x == 100) && tid == 0) printf("ring blk %d grp %d: entry->loop end %lld, ->exit %lld\n", (int)blockIdx.x, grp, t_loop_end_ - t_entry_, clock64() - t_entry_);
+#endif
 }
 
 template <typename T, int N, int MODE, int SIGN, int MAXT>

@@ -40,6 +40,7 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
     C *stw = reinterpret_cast<C *>(smem_raw);
     C *bufs = stw + TWP;
     unsigned long long *full = reinterpret_cast<unsigned long long *>(bufs + (size_t)a.NB * a.bufstride);
+    volatile int *ktile = reinterpret_cast<volatile int *>(full + a.NB);  // as in ring_kernel
 
     const int TL = a.TL, GT = a.GT, G = a.G, NB = a.NB;
     const int grp = threadIdx.x / GT;
@@ -65,6 +66,7 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
     };
 
     if (threadIdx.x == 0) {
+        ktile[NB] = NB;
         for (int b = 0; b < NB; ++b) mbar_init(&full[b], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -76,18 +78,29 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
     // every group owns NBG = NB / G buffers: its leader fills them, its threads consume them, so a buffer's
     // mbarrier never sees a waiter that is not in step with its fills
     const int NBG = NB / G;
+    auto refill = [&](int kn, int b) {
+        if (kn < nloc) {
+            ktile[b] = kn;
+            issue(kn, b);
+        } else {
+            ktile[b] = -1;
+            mbar_arrive(&full[b]);
+        }
+    };
     if (tid == 0)
-        for (int j = 0; j < NBG && grp + j * G < nloc; ++j) issue(grp + j * G, grp * NBG + j);
+        for (int j = 0; j < NBG; ++j) refill(grp * NBG + j, grp * NBG + j);
 
-    for (int k = grp, j = 0; k < nloc; k += G, ++j) {
+    for (int j = 0;; ++j) {
         const int b = grp * NBG + j % NBG;
+        mbar_wait(&full[b], (unsigned)((j / NBG) & 1));
+        const int k = ktile[b];
+        if (k < 0) break;
         C *buf = bufs + (size_t)b * a.bufstride;
         C *dense = buf + (size_t)c * N * TL + t;     // TMA layout [CC][N][TL]: row r of this line at dense[r * TL]
         C *sl = buf + (c * TL + t) * a.pitch;        // exchange layout: padded lines
         const int tile = tile_of(k);
         const int line = (tile % a.tiles_per_outer) * TL + t;  // line index on the non-line axes (within a component)
 
-        mbar_wait(&full[b], (unsigned)((j / NBG) & 1));
         C x[16];
         if constexpr (SMODE == SMODE_DIT) {
 #pragma unroll
@@ -146,10 +159,9 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
                 for (int j = 0; j < nbox; ++j)
                     tma_store_3d(&tmap, 2 * i0, j * a.box_rows, CC > 1 ? cc : o, buf + (size_t)(cc * N + j * a.box_rows) * TL);
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-            if (k + NBG * G < nloc) {
-                bulk_wait_read();
-                issue(k + NBG * G, b);
-            }
+            const int kn = atomicAdd(const_cast<int *>(&ktile[NB]), 1);
+            if (kn < nloc) bulk_wait_read();
+            refill(kn, b);
         }
     }
     if (tid == 0) bulk_wait_all();
