@@ -855,15 +855,12 @@ void choose_groups(const sso_plan *plan, int GT, int bmax, long long tiles_per_c
     if (GT % 32 == 0) {
         const int cap = plan->opt_maxt ? plan->opt_maxt : 512;
         const int gthr = cap / GT > 15 ? 15 : cap / GT;
-        const int g2 = gthr < bmax / 2 ? gthr : bmax / 2;  // double-buffered groups
-        const int g1 = gthr < bmax ? gthr : bmax;          // single-buffered groups
-        if (g2 >= 3 || g2 >= g1) {
-            g = g2;
-            nbg = 2;
-        } else {
-            g = g1;
-            nbg = 1;
-        }
+        // as many groups as threads and buffers allow (measured: four single-buffered groups beat three
+        // double-buffered ones now that a buffer is refilled before its tile's last stage), then a second buffer
+        // per group if there is room
+        g = gthr < bmax ? gthr : bmax;
+        if (g < 1) g = 1;
+        nbg = bmax / g >= 2 ? 2 : 1;
         if (plan->opt_ring > 0) nbg = plan->opt_ring;
         if (plan->opt_groups > 0) g = plan->opt_groups;
         while (g > 1 && (g * GT > cap || g * nbg > bmax)) --g;
@@ -1027,6 +1024,10 @@ int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long 
         plan->tmap_tl[axis] = sh.TL;
     }
     SRingArgs a{};
+    a.psi = psi;
+    a.inner = g.inner;
+    a.comp_stride = plan->npts;
+    a.direct_store = (sh.TL * esz >= 64 && !(plan->dbg_skip & 512)) ? 1 : 0;
     a.tw = A.tw;
     a.TL = sh.TL;
     a.pitch = sh.pitch;

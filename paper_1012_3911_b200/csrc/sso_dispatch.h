@@ -100,6 +100,10 @@ using RingLaunchFn = cudaError_t (*)(const RingArgs &, unsigned threads, size_t 
 // strided-axis passes through the same ring, tiles moved as TMA tensor boxes (sso_sring.cuh)
 enum : int { SMODE_KS = 0, SMODE_KD2 = 1, SMODE_KD4 = 2, SMODE_DIF = 3, SMODE_DIT = 4 };
 struct SRingArgs {
+    void *psi;                // device base of psi (stores from registers; loads go through the tensor map)
+    long long inner;          // element stride along the line
+    long long comp_stride;    // elements between components
+    int direct_store;         // rows are >= 64 bytes: results are stored from registers, not through the buffer
     const void *tw;           // twiddle blocks of the line axis
     int ntiles;               // tiles of TL adjacent lines (x all components when they are independent)
     int TL;                   // adjacent lines per tile: one row of a tile is TL complex numbers, contiguous in memory

@@ -144,24 +144,40 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
         if constexpr (SMODE != SMODE_DIF) DitChain<T, N, LAST, +1>::run(x, u, stw, sl, gb);
 
         gsync(gb);  // every thread of the group is done with the exchange layout
-        if constexpr (SMODE == SMODE_DIF) {
+        if (a.direct_store) {
+            // rows of >= 64 bytes: store from registers (a warp instruction writes 32/TL rows of TL*16 bytes) and
+            // refill the buffer at once
+            if (tid == 0) refill(atomicAdd(const_cast<int *>(&ktile[NB]), 1), b);
+            const long long o = tile / a.tiles_per_outer;
+            const long long i0 = (long long)(tile % a.tiles_per_outer) * TL;
+            C *gout = reinterpret_cast<C *>(a.psi) + (CC > 1 ? (long long)c * a.comp_stride : o * (long long)N * a.inner) + i0 + t;
+            if constexpr (SMODE == SMODE_DIF) {
 #pragma unroll
-            for (int q = 0; q < 16; ++q) dense[(u * 16 + q) * TL] = x[q];
+                for (int q = 0; q < 16; ++q) st_stream(gout + (long long)(u * 16 + q) * a.inner, x[q]);
+            } else {
+#pragma unroll
+                for (int q = 0; q < 16; ++q) st_stream(gout + (long long)(u + q * U) * a.inner, x[q]);
+            }
         } else {
+            if constexpr (SMODE == SMODE_DIF) {
 #pragma unroll
-            for (int q = 0; q < 16; ++q) dense[(u + q * U) * TL] = x[q];
-        }
-        fence_async_smem();
-        gsync(gb);
-        if (tid == 0) {
-            const int o = tile / a.tiles_per_outer, i0 = (tile % a.tiles_per_outer) * TL;
-            for (int cc = 0; cc < CC; ++cc)
-                for (int j = 0; j < nbox; ++j)
-                    tma_store_3d(&tmap, 2 * i0, j * a.box_rows, CC > 1 ? cc : o, buf + (size_t)(cc * N + j * a.box_rows) * TL);
-            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-            const int kn = atomicAdd(const_cast<int *>(&ktile[NB]), 1);
-            if (kn < nloc) bulk_wait_read();
-            refill(kn, b);
+                for (int q = 0; q < 16; ++q) dense[(u * 16 + q) * TL] = x[q];
+            } else {
+#pragma unroll
+                for (int q = 0; q < 16; ++q) dense[(u + q * U) * TL] = x[q];
+            }
+            fence_async_smem();
+            gsync(gb);
+            if (tid == 0) {
+                const int o = tile / a.tiles_per_outer, i0 = (tile % a.tiles_per_outer) * TL;
+                for (int cc = 0; cc < CC; ++cc)
+                    for (int j = 0; j < nbox; ++j)
+                        tma_store_3d(&tmap, 2 * i0, j * a.box_rows, CC > 1 ? cc : o, buf + (size_t)(cc * N + j * a.box_rows) * TL);
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                const int kn = atomicAdd(const_cast<int *>(&ktile[NB]), 1);
+                if (kn < nloc) bulk_wait_read();
+                refill(kn, b);
+            }
         }
     }
     if (tid == 0) bulk_wait_all();
