@@ -103,7 +103,7 @@ struct SRingArgs {
     void *psi;                // device base of psi (stores from registers; loads go through the tensor map)
     long long inner;          // element stride along the line
     long long comp_stride;    // elements between components
-    int direct_store;         // rows are >= 64 bytes: results are stored from registers, not through the buffer
+    int direct_store;         // results are stored from registers (default) instead of through the buffer with a TMA store
     const void *tw;           // twiddle blocks of the line axis
     int ntiles;               // tiles of TL adjacent lines (x all components when they are independent)
     int TL;                   // adjacent lines per tile: one row of a tile is TL complex numbers, contiguous in memory

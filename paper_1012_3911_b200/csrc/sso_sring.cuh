@@ -145,8 +145,8 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
 
         gsync(gb);  // every thread of the group is done with the exchange layout
         if (a.direct_store) {
-            // rows of >= 64 bytes: store from registers (a warp instruction writes 32/TL rows of TL*16 bytes) and
-            // refill the buffer at once
+            // store from registers (a warp instruction writes 32/TL rows of TL complex numbers) and refill the
+            // buffer at once
             if (tid == 0) refill(atomicAdd(const_cast<int *>(&ktile[NB]), 1), b);
             const long long o = tile / a.tiles_per_outer;
             const long long i0 = (long long)(tile % a.tiles_per_outer) * TL;
