@@ -50,6 +50,23 @@ cudaError_t launch_pass(const PassArgs &a, unsigned threads, size_t smem, cudaSt
     return cudaGetLastError();
 }
 
+// Programmatic dependent launch: the CTAs of a pass may start (twiddle copy, barrier setup) while the previous
+// pass of the stream drains; they wait in the kernel (griddepcontrol.wait) before touching psi.
+template <typename K, typename... Args>
+static cudaError_t launch_pdl(K kern, unsigned grid, unsigned threads, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+
 template <typename T, int N, int MODE, int SIGN, int MAXT>
 cudaError_t launch_ring(const RingArgs &a, unsigned threads, size_t smem, unsigned grid, cudaStream_t st) {
     auto kern = ring_kernel<T, N, MODE, SIGN, MAXT>;
@@ -60,8 +77,7 @@ cudaError_t launch_ring(const RingArgs &a, unsigned threads, size_t smem, unsign
         attr_done = true;
     }
     if (threads > (unsigned)MAXT) return cudaErrorInvalidConfiguration;
-    kern<<<grid, threads, smem, st>>>(a);
-    return cudaGetLastError();
+    return launch_pdl(kern, grid, threads, smem, st, a);
 }
 
 template <typename T, int N, int SMODE>
@@ -74,8 +90,7 @@ cudaError_t launch_sring(const SRingArgs &a, const void *tensor_map, unsigned th
         attr_done = true;
     }
     if (threads > 512u) return cudaErrorInvalidConfiguration;
-    kern<<<grid, threads, smem, st>>>(a, *reinterpret_cast<const CUtensorMap *>(tensor_map));
-    return cudaGetLastError();
+    return launch_pdl(kern, grid, threads, smem, st, a, *reinterpret_cast<const CUtensorMap *>(tensor_map));
 }
 
 #define SSO_CAT3_(a, b, c) a##b##_##c

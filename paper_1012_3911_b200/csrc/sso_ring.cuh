@@ -153,6 +153,8 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
             prefetch_l2_bulk_plain(reinterpret_cast<const char *>(a.vtab) + (size_t)l0 * N * vesz, (unsigned)(TL * N * vesz));
     };
 
+    // let the next pass of the stream start its own setup as SMs free up
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (threadIdx.x == 0) {
         ktile[NB] = NB;
         for (int b = 0; b < NB; ++b) mbar_init(&full[b], 1);
@@ -163,6 +165,8 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
         for (int i = threadIdx.x; i < TWN; i += blockDim.x) stw[i] = gtw[i];
     }
     __syncthreads();
+    // everything above touched only plan-owned tables; psi is valid once the previous pass has completed
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     // every group owns NBG = NB / G buffers: its leader fills them, its threads consume them, so a buffer's
     // mbarrier never sees a waiter that is not in step with its fills
     const int NBG = NB / G;

@@ -65,6 +65,8 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
                 tma_load_3d(dst + (size_t)(cc * N + j * a.box_rows) * TL, &tmap, 2 * i0, j * a.box_rows, CC > 1 ? cc : o, &full[b]);
     };
 
+    // let the next pass of the stream start its own setup as SMs free up
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (threadIdx.x == 0) {
         ktile[NB] = NB;
         for (int b = 0; b < NB; ++b) mbar_init(&full[b], 1);
@@ -75,6 +77,8 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
         for (int i = threadIdx.x; i < TWN; i += blockDim.x) stw[i] = gtw[i];
     }
     __syncthreads();
+    // everything above touched only plan-owned tables; psi is valid once the previous pass has completed
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     // every group owns NBG = NB / G buffers: its leader fills them, its threads consume them, so a buffer's
     // mbarrier never sees a waiter that is not in step with its fills
     const int NBG = NB / G;
