@@ -232,14 +232,16 @@ template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void di
 // barrier over one group of a CTA (groups are independent pipelines that share only the twiddle table):
 // gb = 0 means the CTA holds one group (plain __syncthreads), otherwise gb = (named barrier id) | (threads << 8)
 __device__ __forceinline__ void gsync(int gb) {
-    if ((gb & 0x3fffffff) == 0) __syncthreads();
-    else asm volatile("bar.sync %0, %1;" ::"r"(gb & 15), "r"((gb & 0x3fffffff) >> 8) : "memory");
+    if ((gb & 0x03ffffff) == 0) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(gb & 15), "r"((gb & 0x03ffffff) >> 8) : "memory");
 }
 
 // gb flag: consecutive lanes hold consecutive u of one line (contiguous-axis kernels).  The exchange between
 // two stages only moves data inside blocks of max(Mi) consecutive u (Mi = sub-transform length / 16), so when
 // such a block lies inside a warp the group barrier shrinks to a __syncwarp
 constexpr int GB_LANES_ARE_U = 1 << 30;
+// strided kernels interleave TL lines in a warp (lane = u * TL + t): bits 26..29 hold log2(TL)
+constexpr int GB_TL_SHIFT = 26;
 
 // registers (layout of stage IA) -> shared memory -> registers (layout of stage IB)
 template <typename T, int N, int IA, int IB> __device__ __forceinline__ void exchange(typename CxOf<T>::type (&x)[16], int u, typename CxOf<T>::type *sl, int gb) {
@@ -248,7 +250,7 @@ template <typename T, int N, int IA, int IB> __device__ __forceinline__ void exc
     constexpr int SCOPE = MiA > MiB ? MiA : MiB;
     C *wa = sl + stage_base<N, IA>(u);
     const C *rb = sl + stage_base<N, IB>(u);
-    const bool warp_local = SCOPE <= 32 && (gb & GB_LANES_ARE_U);
+    const bool warp_local = (gb & GB_LANES_ARE_U) && (SCOPE << ((gb >> GB_TL_SHIFT) & 15)) <= 32;
     if (warp_local) __syncwarp();
     else gsync(gb);
 #pragma unroll

@@ -45,7 +45,8 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
     const int TL = a.TL, GT = a.GT, G = a.G, NB = a.NB;
     const int grp = threadIdx.x / GT;
     const int tid = threadIdx.x - grp * GT;
-    const int gb = G > 1 ? ((grp + 1) | (GT << 8)) : 0;
+    // lane = u * TL + t within a component: exchanges confined to 32 / TL consecutive u stay inside a warp
+    const int gb = (G > 1 ? ((grp + 1) | (GT << 8)) : 0) | ((32 % TL == 0 && (U * TL) % 32 == 0) ? (GB_LANES_ARE_U | ((31 - __clz(TL)) << GB_TL_SHIFT)) : 0);
     const int t = tid % TL;
     const int cu = tid / TL;
     const int u = cu % U;
@@ -113,6 +114,8 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
 #pragma unroll
             for (int q = 0; q < 16; ++q) x[q] = dense[(u + q * U) * TL];
         }
+
+        gsync(gb);  // the exchange layout overlaps the TMA layout of other warps' lines
 
         if constexpr (SMODE != SMODE_DIT) DifChain<T, N, 0, -1>::run(x, u, stw, sl, gb);
 
