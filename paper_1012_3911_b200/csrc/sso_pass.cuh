@@ -394,7 +394,7 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
     const int GT = a.GT;
     const int grp = threadIdx.x / GT;
     const int tid = threadIdx.x - grp * GT;
-    const int gb = a.G > 1 ? ((grp + 1) | (GT << 8)) : 0;
+    const int gb = (a.G > 1 ? ((grp + 1) | (GT << 8)) : 0) | ((!STRIDED && (U >= 32 || 32 % U == 0)) ? GB_LANES_ARE_U : 0);
     int t, c, u;
     if (STRIDED) {
         t = tid % TL;

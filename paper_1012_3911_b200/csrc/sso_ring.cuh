@@ -1,19 +1,20 @@
 // sso_ring.cuh -- the contiguous-axis pass of a 2D/3D lattice as an asynchronous ring pipeline (sm_100a).
 //
 // The last lattice axis is contiguous in memory, so a tile of TL whole lines is one contiguous block.  One
-// persistent CTA per SM owns a ring of NB shared-memory buffers.  Tiles are moved by the bulk-copy engine
-// (cp.async.bulk, SASS UBLKCP): global -> buffer, completion signalled on an mbarrier, and buffer -> global
-// as a bulk store.  G independent groups of GT threads each take the tiles of the ring in turn, and, with the
-// tile in registers (16 points per thread) and its buffer as the exchange area, apply
+// persistent CTA per SM owns a set of shared-memory buffers.  A tile is fetched by the bulk-copy engine
+// (cp.async.bulk, SASS UBLKCP) onto an mbarrier.  G independent groups of GT threads, each with its own
+// buffers, take tiles as they become free and, with the tile in registers (16 points per thread) and its
+// buffer as the exchange area, apply
 //
 //   MODE_OPEN   V/2 (natural order)  ->  forward DIF  ->  natural frequency order
 //   MODE_MID    inverse DIF  ->  merged potential phase V (permuted order)  ->  forward DIT
 //   MODE_CLOSE  inverse DIF  ->  natural order  ->  V/2
 //
-// (eq. 7, 98 eq. 11; the FFT stages are those of sso_pass.cuh).  No thread ever waits for HBM
-// with work in its registers: the load of the tile that will reuse a buffer is issued as soon as that
-// buffer's store has been read out, NB tiles ahead of its use, and the potential-phase lines of that tile
-// are requested into L2 at the same time.
+// (eq. 7, 98 eq. 11; the FFT stages are those of sso_pass.cuh).  As soon as the last exchange of a
+// tile has been read, the group's leader claims the next tile of the CTA, refills the buffer and asks L2 for
+// that tile's potential-phase lines; the results are stored from registers (512 contiguous bytes per warp
+// instruction).  The pass is launched with programmatic dependent launch: its setup overlaps the drain of the
+// previous pass of the stream, and it waits (griddepcontrol.wait) before it touches psi.
 #pragma once
 #include <cstdio>
 
