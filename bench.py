@@ -53,7 +53,12 @@ DESCR = {
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per pass-kernel launch from the committed `ncu --set full`
 # capture (profiles/, see the .md beside each); None where no capture exists yet
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    # profiles/r1e_final.md: mean over the pass kernels of one steady-state step
+    "2a": 0.5 * (153.5e6 + 85.5e6),
+    "3": 0.25 * (476.4e6 + 478.5e6 + 475.3e6 + 753.8e6),
+    "5": 0.25 * (2458e6 + 2085e6 + 2091e6 + 2085e6),
+}
 
 
 def load_peaks():
@@ -277,7 +282,7 @@ def run_product(args):
                        "l2": "no flush: psi + potential phase table streamed per split step = %.0f MB (L2 is 126 MB)" % (2 * S / 1e6 if name != "2b" else 2 * S / 1e6),
                        "norm_after": norm_after},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
-                         "kernel": "sso::pass_kernel", "bytes_per_launch": bytes_per_launch, "avg_launch_us": per_launch_s * 1e6,
+                         "kernel": ("sso::ring_kernel + sso::sring_kernel (every pass launch moves psi once; average over the step's pass launches)" if len(w.sizes) > 1 else "sso::pass_kernel (one persistent CTA, psi stays on the SM)"), "bytes_per_launch": bytes_per_launch, "avg_launch_us": per_launch_s * 1e6,
                          "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": S, "d2h_bytes_per_step": S, "norm_after": e2e_norm},
             "gpu_launches": int(launches_per_call * K),
