@@ -1,25 +1,33 @@
 #!/usr/bin/env python
 """bench.py -- grid-point updates/s of the Fourier split-operator step on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 2a] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 5] [--only] [--impl reference]
 
 One bench "step" is one pass of the whole hot path over one batch: a single call of
 sso_step(psi, SPLIT_STEPS) that advances the wavefunction by SPLIT_STEPS = 128 split-operator time steps
 (the paper's protocol: 128 time steps, one upload before and one download after).
+
+Headline workload at N=1: BASELINE.json's metric is not quoted on one config, so the line's top-level numbers are
+for the LARGEST single-GPU configuration, config 5 (3D Dirac, 4 x 256^3 complex128, 1 GiB of psi); the other
+five workloads (1, 2a, 2b, 3, 4) are timed in the same run and reported under config.per_workload.
   value  device-resident throughput: psi, the potential table and the field table are in HBM before the
          timed region; K calls timed with CUDA events on the launching stream.
   e2e    the same K calls through sso_step_host on a pinned HOST buffer: every call uploads psi, steps and
          downloads it inside the timed region.
   roofline  HBM: algorithmic bytes of one pass-kernel launch (one read + one write of psi, DESIGN.md
-         "Bytes") / average pass-kernel launch duration over the timed region, against MEASURED_PEAKS.json.
-  cpu_baseline  the oracle as it stands on the host cores, bounded sample, rank 0 at N=1 only.
-Workload at N=1: BASELINE.json configs[1], complex128 ("2a": 2D Schroedinger 2048^2 with a dipole field).
-N>1: replicas only: every rank runs the same workload on its own GPU, no
+         "Rooflines") / average pass-kernel launch duration over the timed region, against MEASURED_PEAKS.json;
+         `per_pass` = the same for each pass kind of one split step, timed with CUDA events by the library
+         (sso_profile_step); `traffic` = ncu DRAM bytes of the dominant kernel from profiles/traffic.json, or
+         null when csrc/ has changed since that capture.
+  cpu_baseline  the oracle as it stands on the host cores (all cores, and one thread), bounded samples, rank 0
+         at N=1 only.
+N>1: replicas only: every rank runs the headline workload on its own GPU, no
 data-path collective; value = all ranks' updates / max-over-ranks time.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import subprocess
@@ -38,6 +46,7 @@ import workloads as wl  # noqa: E402
 METRIC = "grid-point updates/s per split-operator step"
 UNIT = "grid-point updates/s"
 SPLIT_STEPS = 128  # split-operator steps per sso_step call ("over 128 time steps")
+HEADLINE = "5"
 
 # name -> (config number, precision name, passes P per steady-state step)
 WORKLOADS = {
@@ -51,14 +60,8 @@ DESCR = {
     "4": "cfg4 2D Dirac 2 components 1024x1024, soft-core Coulomb + A(t) in the kinetic unitary, complex128",
     "5": "cfg5 3D Dirac 4 components 256^3, soft-core Coulomb, complex128",
 }
-# dram__bytes_read.sum + dram__bytes_write.sum per pass-kernel launch from the committed `ncu --set full`
-# capture (profiles/, see the .md beside each); None where no capture exists yet
-NCU_TRAFFIC_BYTES = {
-    # profiles/r1e_final.md: mean over the pass kernels of one steady-state step
-    "2a": 0.5 * (153.5e6 + 85.5e6),
-    "3": 0.25 * (476.4e6 + 478.5e6 + 475.3e6 + 753.8e6),
-    "5": 0.25 * (2458e6 + 2085e6 + 2091e6 + 2085e6),
-}
+# 60 % of the 8 TB/s roofline, us per split step; None where the bar does not apply
+BAR_US = {"1": None, "2a": 55.9, "2b": 28.0, "3": 447.4, "4": 28.0, "5": 1789.6}
 
 
 def load_peaks():
@@ -69,6 +72,31 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def csrc_sha() -> str:
+    """Hash of the kernel sources: an ncu number is only quoted while the code it was taken from is unchanged."""
+    h = hashlib.sha256()
+    for p in sorted((ROOT / "paper_1012_3911_b200" / "csrc").glob("*")):
+        if p.suffix in (".cu", ".cuh", ".h"):
+            h.update(p.name.encode())
+            h.update(p.read_bytes())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(name: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed capture
+    listed in profiles/traffic.json -- or None when there is no capture for this workload or csrc/ has changed."""
+    p = ROOT / "profiles" / "traffic.json"
+    if not p.exists():
+        return None, "no profiles/traffic.json"
+    d = json.loads(p.read_text())
+    if d.get("csrc_sha16") != csrc_sha():
+        return None, f"stale: {d.get('capture')} was taken at csrc {d.get('csrc_sha16')}, csrc is now {csrc_sha()}"
+    e = d.get("workloads", {}).get(name)
+    if not e:
+        return None, "no capture for this workload"
+    return float(e["dram_bytes_per_launch"]), f"{d.get('capture')}: {e.get('kernel')}"
+
+
 def make_workload(name: str, nrows: int):
     cfg, prec, P = WORKLOADS[name]
     w = wl.CONFIGS[cfg](nsteps=nrows)
@@ -76,7 +104,7 @@ def make_workload(name: str, nrows: int):
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed regions (B200_PROFILING.md)."""
 
     Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
@@ -89,6 +117,7 @@ class ClockSampler:
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thr = threading.Thread(target=self._read, daemon=True)
             self.thr.start()
+            time.sleep(0.15)
         except OSError:
             self.proc = None
 
@@ -96,12 +125,13 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), line.strip()))
 
-    def stop(self, t0: float, t1: float):
+    def window(self, t0: float, t1: float):
+        """Summary of the samples taken in [t0, t1] (plus one on each side for regions shorter than the period)."""
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.12)
-        self.proc.terminate()
-        inside = [r for t, r in self.rows if t0 <= t <= t1] or [r for _, r in self.rows[-3:]]
+        rows = list(self.rows)
+        inside = [r for t, r in rows if t0 <= t <= t1] or [r for t, r in rows if t0 - 0.1 <= t <= t1 + 0.1] or [r for _, r in rows[-2:]]
         mhz, mx, reasons = [], None, set()
         for r in inside:
             f = [x.strip() for x in r.split(",")]
@@ -117,24 +147,37 @@ class ClockSampler:
                     reasons.add(nm)
         return {"sm_mhz": float(np.median(mhz)) if mhz else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(mhz)}
 
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
 
-def oracle_rate(w, seconds_target: float = 12.0):
-    """The oracle as it stands, all host cores it uses, on a bounded sample of split steps of the same workload."""
+
+def oracle_rate(w, seconds_target: float, threads: int | None = None):
+    """The oracle as it stands on a bounded sample of split steps of the same full-size workload."""
     import oracle
 
-    o = oracle.Solver(w.sizes, w.dx, w.dt, w.ncomp, w.mass, w.c, w.charge)
-    o.set_potential(w.V)
-    if w.field_kind:
-        o.set_field(w.field_kind, w.step_avg)
-    psi = w.psi0
-    t0 = time.perf_counter()
-    psi = o.step(psi, 1)
-    one = time.perf_counter() - t0
-    n = int(max(1, min(w.step_avg.shape[0] - 1 if w.field_kind else 10**9, seconds_target / max(one, 1e-6))))
-    t0 = time.perf_counter()
-    o.step(psi, n)
-    dt = time.perf_counter() - t0
-    return w.npoints * n / dt, n, oracle.max_threads(), dt
+    allc = oracle.max_threads()
+    if threads:
+        oracle.set_threads(threads)
+    try:
+        o = oracle.Solver(w.sizes, w.dx, w.dt, w.ncomp, w.mass, w.c, w.charge)
+        o.set_potential(w.V)
+        if w.field_kind:
+            o.set_field(w.field_kind, w.step_avg)
+        psi = w.psi0
+        t0 = time.perf_counter()
+        psi = o.step(psi, 1)
+        one = time.perf_counter() - t0
+        n = int(max(1, min(w.step_avg.shape[0] - 1 if w.field_kind else 10**9, (seconds_target - one) / max(one, 1e-6))))
+        if seconds_target - one < one:  # the first step already used the budget: it is the sample
+            return w.npoints / one, 1, threads or allc, one
+        t0 = time.perf_counter()
+        o.step(psi, n)
+        dt = time.perf_counter() - t0
+        return w.npoints * n / dt, n, threads or allc, dt
+    finally:
+        if threads:
+            oracle.set_threads(allc)
 
 
 def run_reference(args):
@@ -187,35 +230,18 @@ def job_throughput(updates_per_rank: float, ms_local: float, world: int, device:
     return updates_per_rank * world / (ms * 1e-3), ms
 
 
-def run_product(args):
+def measure(name, K, W, world, barrier, sampler, want_e2e):
+    """Time K calls of sso_step(psi, 128) of one workload.  Returns (record, workload)."""
     import torch
-    import torch.distributed as dist
 
     import paper_1012_3911_b200 as sso
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    name = args.workload
-    K, W = args.steps, args.warmup
-    nrows = SPLIT_STEPS  # every call replays field rows 0..127 (sso_set_time_index(0) before each call)
-    w, prec, P = make_workload(name, nrows)
+    w, prec, P = make_workload(name, SPLIT_STEPS)  # every call replays field rows 0..127
     precision = sso.C128 if prec == "c128" else sso.C64
     cdt = np.complex128 if prec == "c128" else np.complex64
     esz = 16 if prec == "c128" else 8
     S = w.npoints * w.ncomp * esz
+    nd = len(w.sizes)
 
     plan = sso.Plan(w.sizes, w.dx, w.dt, w.ncomp, precision)
     plan.set_constants(w.mass, w.c, w.charge)
@@ -230,13 +256,9 @@ def run_product(args):
         plan.set_time_index(0)
         plan.step(psi, SPLIT_STEPS, stream=stream)
 
-    for _ in range(max(W, 3) if W else 0):
+    for _ in range(max(W, 3)):
         call()
     launches_per_call = plan.launch_count(SPLIT_STEPS)
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-        time.sleep(0.15)
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0 = time.time()
@@ -246,54 +268,121 @@ def run_product(args):
     e1.record(stream)
     barrier()
     t1 = time.time()
-    ms = e0.elapsed_time(e1)
+    ms_local = e0.elapsed_time(e1)
     norm_after = plan.norm(psi)
-    value, ms = job_throughput(float(w.npoints) * SPLIT_STEPS * K, ms, world)
-    clocks = sampler.stop(t0, t1) if rank == 0 else None
+    value, ms = job_throughput(float(w.npoints) * SPLIT_STEPS * K, ms_local, world)
+    clocks = sampler.window(t0, t1) if sampler else None
 
-    # end to end: host buffer in, host buffer out, copies inside the timed region
-    host = torch.from_numpy(psi0.copy()).pin_memory()
-    for _ in range(2):
+    peak, peak_src = load_peaks()
+    us_step = ms * 1e3 / (K * SPLIT_STEPS)
+    pass_launches = K * (SPLIT_STEPS * P + 1) if nd > 1 else K
+    per_launch_s = ms * 1e-3 / pass_launches
+    bytes_per_launch = 2.0 * S  # one read + one write of psi
+    achieved = bytes_per_launch / per_launch_s / 1e9
+    rec = {
+        "workload": DESCR[name], "grid": list(w.sizes), "ncomp": w.ncomp, "dtype": "f64" if prec == "c128" else "f32",
+        "us_per_split_step": us_step, "updates_per_s": value, "ms_per_call": ms / K, "passes_per_split_step": P if nd > 1 else 0,
+        "achieved_GBs": achieved, "frac_of_measured": achieved / peak, "frac_of_8TBs": achieved / 8000.0,
+        "bar_us_per_split_step": BAR_US[name], "meets_60pct_of_8TBs": (us_step <= BAR_US[name]) if BAR_US[name] else None,
+        "norm_after": norm_after, "clocks": clocks, "gpu_launches": int(launches_per_call * K),
+        "l2": ("psi larger than L2: every pass streams it from HBM" if S > 126e6 else
+               "psi (%.0f MB) fits L2 (126 MB): consecutive passes of a step sequence re-touch it there; no flush, ncu DRAM bytes are below the algorithmic bytes" % (S / 1e6)),
+    }
+    if nd == 1:
+        rec["note"] = "one persistent CTA, psi stays on the SM for all 128 steps: the HBM figure is 2S per CALL over the call time, not a roofline (SURVEY H5)"
+        rec["achieved_GBs"] = rec["frac_of_measured"] = rec["frac_of_8TBs"] = None
+    # per pass kind, one profiled split-step sequence (events between the passes: no overlap between passes)
+    try:
         plan.set_time_index(0)
-        plan.step_host(host, SPLIT_STEPS)
-    host.copy_(torch.from_numpy(psi0))
-    barrier()
-    h0 = time.perf_counter()
-    for _ in range(K):
-        plan.set_time_index(0)
-        plan.step_host(host, SPLIT_STEPS)  # synchronous: returns after the download
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - h0
-    e2e_value, _ = job_throughput(float(w.npoints) * SPLIT_STEPS * K, e2e_s * 1e3, world)
-    e2e_norm = float(np.sum(np.abs(host.numpy().astype(np.complex128)) ** 2) * np.prod(w.dx))
+        rec["per_pass"] = [{"pass": n_, "launches": c_, "avg_us": t_, "achieved_GBs": (bytes_per_launch / (t_ * 1e-6) / 1e9 if t_ > 0 else None)}
+                           for n_, c_, t_ in plan.profile_step(psi, 8, stream=stream)]
+    except AttributeError:
+        pass
+    e2e = None
+    if want_e2e:
+        host = torch.from_numpy(psi0.copy()).pin_memory()
+        for _ in range(2):
+            plan.set_time_index(0)
+            plan.step_host(host, SPLIT_STEPS)
+        host.copy_(torch.from_numpy(psi0))
+        barrier()
+        h0 = time.perf_counter()
+        for _ in range(K):
+            plan.set_time_index(0)
+            plan.step_host(host, SPLIT_STEPS)  # synchronous: returns after the download
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - h0
+        e2e_value, _ = job_throughput(float(w.npoints) * SPLIT_STEPS * K, e2e_s * 1e3, world)
+        e2e_norm = float(np.sum(np.abs(host.numpy().astype(np.complex128)) ** 2) * np.prod(w.dx))
+        e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": S, "d2h_bytes_per_step": S, "norm_after": e2e_norm}
+        del host
+    plan.destroy()
+    del psi
+    torch.cuda.empty_cache()
+    return rec, e2e, w, (ms, bytes_per_launch, per_launch_s, achieved, peak, peak_src)
+
+
+def run_product(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.gpus != world:
+        raise SystemExit(f"bench.py --gpus {args.gpus} but WORLD_SIZE={world}: launch N>1 with torch.distributed.run (one rank per GPU)")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    K, W = args.steps, args.warmup
+    head = args.workload
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    rec, e2e, w, (ms, bytes_per_launch, per_launch_s, achieved, peak, peak_src) = measure(head, K, W, world, barrier, sampler, True)
+    per = {head: rec}
+    if world == 1 and not args.only:
+        for name in WORKLOADS:
+            if name != head:
+                per[name] = measure(name, min(K, 10), W, world, barrier, sampler, False)[0]
+    if sampler:
+        sampler.stop()
 
     if rank == 0:
-        peak, peak_src = load_peaks()
-        pass_launches = K * (SPLIT_STEPS * P + (1 if len(w.sizes) > 1 else 0)) if len(w.sizes) > 1 else K
-        per_launch_s = ms * 1e-3 / pass_launches
-        bytes_per_launch = 2.0 * S if len(w.sizes) > 1 else 2.0 * S  # one read + one write of psi
-        achieved = bytes_per_launch / per_launch_s / 1e9
-        traffic = NCU_TRAFFIC_BYTES.get(name)
+        traffic, traffic_src = ncu_traffic(head)
+        nd = len(w.sizes)
+        dominant = max(rec.get("per_pass", []), key=lambda r: r["avg_us"] * r["launches"], default=None)
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if prec == "c128" else "f32", "data": "synthetic",
-            "config": {"workload": DESCR[name], "split_steps_per_step": SPLIT_STEPS, "grid": list(w.sizes), "ncomp": w.ncomp,
-                       "parallelism": "replicas" if world > 1 else "single GPU", "us_per_split_step": ms * 1e3 / (K * SPLIT_STEPS),
-                       "l2": "no flush: psi + potential phase table streamed per split step = %.0f MB (L2 is 126 MB)" % (2 * S / 1e6 if name != "2b" else 2 * S / 1e6),
-                       "norm_after": norm_after},
+            "metric": METRIC, "value": rec["updates_per_s"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": rec["dtype"], "data": "synthetic",
+            "config": {"workload": DESCR[head], "split_steps_per_step": SPLIT_STEPS, "grid": list(w.sizes), "ncomp": w.ncomp,
+                       "parallelism": "replicas" if world > 1 else "single GPU", "us_per_split_step": rec["us_per_split_step"],
+                       "l2": rec["l2"], "norm_after": rec["norm_after"], "per_workload": per},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
-                         "kernel": ("sso::ring_kernel + sso::sring_kernel (every pass launch moves psi once; average over the step's pass launches)" if len(w.sizes) > 1 else "sso::pass_kernel (one persistent CTA, psi stays on the SM)"), "bytes_per_launch": bytes_per_launch, "avg_launch_us": per_launch_s * 1e6,
+                         "traffic_source": traffic_src,
+                         "kernel": ("average over the pass launches of a split step (every pass launch moves psi once: sso::ring_kernel on the contiguous axis, sso::sring_kernel on the strided axes); per_pass lists each" if nd > 1 else "sso::pass_kernel (one persistent CTA, psi stays on the SM)"),
+                         "dominant_pass": dominant, "bytes_per_launch": bytes_per_launch, "avg_launch_us": per_launch_s * 1e6,
                          "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": S, "d2h_bytes_per_step": S, "norm_after": e2e_norm},
-            "gpu_launches": int(launches_per_call * K),
-            "clocks": clocks,
+            "e2e": e2e,
+            "gpu_launches": rec["gpu_launches"],
+            "clocks": rec["clocks"],
         }
         if world == 1 and not args.no_cpu_baseline:
-            v, n, cores, secs = oracle_rate(w)
+            v, n, cores, secs = oracle_rate(w, 12.0)
+            v1, n1, _, secs1 = oracle_rate(w, 6.0, threads=1)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "sample": f"{n} split-operator steps of the same full-size workload in {secs:.1f} s (fp64)"}
+                                    "sample": f"{n} split-operator steps of the same full-size workload in {secs:.1f} s (fp64)",
+                                    "single_thread": {"value": v1, "cores": 1, "sample": f"{n1} split-operator step(s) in {secs1:.1f} s"}}
         print(json.dumps(line), flush=True)
-    plan.destroy()
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -305,7 +394,8 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="sso", choices=["sso", "reference"])
-    ap.add_argument("--workload", default="2a", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default=HEADLINE, choices=sorted(WORKLOADS), help="headline workload (top-level numbers)")
+    ap.add_argument("--only", action="store_true", help="time the headline workload only (no per_workload sweep)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

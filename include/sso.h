@@ -68,7 +68,10 @@ extern "C" {
 #define SSO_OPT_LINES_PER_TILE_CONTIG 1  /* lines per CTA in contiguous-axis passes (0 = auto)   */
 #define SSO_OPT_LINES_PER_TILE_STRIDED 2 /* adjacent lines per CTA in strided-axis passes (0=auto) */
 #define SSO_OPT_POTENTIAL_PHASE 3        /* 0 = complex phase table exp(-i V tau/2) (default),
-                                            1 = real angle table + in-kernel sincos polynomial   */
+                                            1 = real angle table + in-kernel sincos.  The plan keeps
+                                            no copy of V: CHANGING this option discards the potential,
+                                            and sso_step fails with SSO_ERR_STATE until
+                                            sso_set_potential has been called again                */
 
 #define SSO_OPT_GROUPS_PER_CTA 4         /* independent line groups per CTA (0 = auto)              */
 #define SSO_OPT_RING_BUFFERS 5           /* ring buffers PER GROUP of the ring pipelines (0 = auto: 2 if they fit) */
@@ -133,7 +136,12 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream);
  */
 int sso_step_host(sso_plan *plan, void *psi_host, int64_t nsteps);
 
-/* *out_host = sum_c sum_r |psi_c(r)|^2 prod(dx), accumulated in double.  Synchronises `stream`. */
+/*
+ * *out_host = sum_c sum_r |psi_c(r)|^2 prod(dx), the lattice form of the norm integral of |psi|^2 that every
+ * factor of the step preserves (the step is a product of unitary factors, eq. 7 and 76 eq. 8; the
+ * paper plots this density).  psi is a DEVICE pointer laid out as for sso_step; the sum is
+ * accumulated in double also for SSO_C64, in a fixed order (deterministic).  Synchronises `stream`.
+ */
 int sso_norm(sso_plan *plan, const void *psi, double *out_host, void *stream);
 
 /* Tuning knobs (SSO_OPT_*); invalid values give SSO_ERR_INVALID. */
@@ -144,6 +152,25 @@ int sso_set_option(sso_plan *plan, int option, int64_t value);
  * current state (for launch accounting in benchmarks).
  */
 int sso_launch_count(const sso_plan *plan, int64_t nsteps, int64_t *count);
+
+/*
+ * Measurement aid: advances psi by nsteps exactly like sso_step, but brackets every pass launch with CUDA
+ * events (which keeps consecutive passes from overlapping) and returns, per pass kind, the number of launches
+ * in count[SSO_PASS_KINDS] and their mean duration in microseconds in mean_us[SSO_PASS_KINDS] (host arrays).
+ * The pass kinds are the passes of the fused step (eq. 8 factor by
+ * factor).  Synchronises `stream`.  sso_pass_name returns a static description of a kind.
+ */
+#define SSO_PASS_OPENING 0        /* V/2 and the forward transform along the last axis            */
+#define SSO_PASS_POTENTIAL 1      /* inverse transform, merged potential phase, forward transform  */
+#define SSO_PASS_CLOSING 2        /* inverse transform along the last axis and V/2                 */
+#define SSO_PASS_KINETIC 3        /* forward transform, kinetic factor, inverse transform (axis 0) */
+#define SSO_PASS_MIDDLE_FORWARD 4 /* 3D: forward transform along the middle axis                   */
+#define SSO_PASS_MIDDLE_INVERSE 5 /* 3D: inverse transform along the middle axis                   */
+#define SSO_PASS_LINE_1D 6        /* 1D: every step of the call in one persistent launch           */
+#define SSO_PASS_TABLES 7         /* small per-step table kernels (field phases, kinetic phases)   */
+#define SSO_PASS_KINDS 8
+int sso_profile_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream, int64_t *count, double *mean_us);
+const char *sso_pass_name(int kind);
 
 /* Frees every table; NULL is a no-op returning SSO_OK. */
 int sso_destroy(sso_plan *plan);

@@ -26,8 +26,9 @@ OPT_LINES_PER_TILE_CONTIG, OPT_LINES_PER_TILE_STRIDED, OPT_POTENTIAL_PHASE = 1, 
 SYMBOLS = (
     "sso_plan_create", "sso_set_constants", "sso_set_potential", "sso_set_field", "sso_set_time_index",
     "sso_get_time_index", "sso_step", "sso_step_host", "sso_norm", "sso_set_option", "sso_launch_count",
-    "sso_destroy", "sso_last_error", "sso_version", "sso_debug_layout",
+    "sso_destroy", "sso_last_error", "sso_version", "sso_debug_layout", "sso_profile_step", "sso_pass_name",
 )
+PASS_KINDS = 8
 
 
 class SsoError(RuntimeError):
@@ -62,8 +63,11 @@ def lib() -> ctypes.CDLL:
         L.sso_last_error.argtypes = [vp]
         L.sso_last_error.restype = ctypes.c_char_p
         L.sso_version.restype = ctypes.c_char_p
+        L.sso_profile_step.argtypes = [vp, vp, i64, vp, ctypes.POINTER(i64), ctypes.POINTER(dbl)]
+        L.sso_pass_name.argtypes = [ci]
+        L.sso_pass_name.restype = ctypes.c_char_p
         for name in SYMBOLS:
-            if name not in ("sso_last_error", "sso_version"):
+            if name not in ("sso_last_error", "sso_version", "sso_pass_name"):
                 getattr(L, name).restype = ci
         _lib = L
     return _lib
@@ -84,6 +88,31 @@ def _ptr(x) -> Optional[int]:
     if hasattr(x, "ctypes"):
         return x.ctypes.data
     raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _check_buffer(x, want_bytes: int, elem_bytes: int, device: Optional[bool], what: str) -> None:
+    """The C ABI takes bare pointers and cannot check them: refuse a tensor/array whose size, element width,
+    contiguity or residence does not match the plan.  Raw integer addresses are the caller's responsibility."""
+    if x is None or isinstance(x, int):
+        return
+    if hasattr(x, "data_ptr"):  # torch tensor
+        if device is not None and bool(x.is_cuda) != device:
+            raise ValueError(f"{what}: expected a {'CUDA' if device else 'host'} tensor")
+        if not x.is_contiguous():
+            raise ValueError(f"{what}: tensor must be contiguous")
+        nbytes, esz = x.numel() * x.element_size(), x.element_size()
+    elif hasattr(x, "ctypes"):  # numpy array
+        if device:
+            raise ValueError(f"{what}: expected a CUDA tensor, got a host array")
+        if not x.flags["C_CONTIGUOUS"]:
+            raise ValueError(f"{what}: array must be C-contiguous")
+        nbytes, esz = x.nbytes, x.itemsize
+    else:
+        return
+    if esz != elem_bytes:
+        raise ValueError(f"{what}: element size {esz} bytes, the plan expects {elem_bytes}")
+    if nbytes != want_bytes:
+        raise ValueError(f"{what}: {nbytes} bytes, the plan expects {want_bytes}")
 
 
 def _stream(s) -> Optional[int]:
@@ -107,6 +136,11 @@ class Plan:
         if rc != OK:
             raise SsoError(rc, L.sso_last_error(None).decode())
         self.sizes, self.ncomp, self.precision = tuple(int(s) for s in sizes), int(ncomp), int(precision)
+        self._npts = 1
+        for n in self.sizes:
+            self._npts *= n
+        self._esz = 16 if self.precision == C128 else 8
+        self._psi_bytes = self._npts * self.ncomp * self._esz
 
     def _ck(self, rc: int) -> None:
         if rc != OK:
@@ -117,6 +151,7 @@ class Plan:
 
     def set_potential(self, V, on_device: bool = False, stream=None) -> None:
         """V: float64 array of shape sizes (numpy on host, or a torch CUDA tensor with on_device=True); None = 0."""
+        _check_buffer(V, self._npts * 8, 8, bool(on_device), "V")
         self._ck(lib().sso_set_potential(self._h, _ptr(V), int(bool(on_device)), _stream(stream)))
 
     def set_field(self, kind: int, step_avg=None) -> None:
@@ -125,6 +160,7 @@ class Plan:
             self._ck(lib().sso_set_field(self._h, int(kind), None, 0))
             return
         nvals = step_avg.shape[0]
+        _check_buffer(step_avg, nvals * len(self.sizes) * 8, 8, False, "step_avg")
         self._ck(lib().sso_set_field(self._h, int(kind), _ptr(step_avg), int(nvals)))
 
     def set_time_index(self, n: int) -> None:
@@ -140,16 +176,27 @@ class Plan:
 
     def step(self, psi, nsteps: int, stream=None) -> None:
         """psi: device buffer (torch CUDA tensor, complex64/complex128, shape (ncomp, *sizes)); in place, asynchronous."""
+        _check_buffer(psi, self._psi_bytes, self._esz, True, "psi")
         self._ck(lib().sso_step(self._h, _ptr(psi), int(nsteps), _stream(stream)))
 
     def step_host(self, psi_host, nsteps: int) -> None:
         """psi_host: host buffer (numpy array or pinned torch tensor); copied up, stepped, copied back."""
+        _check_buffer(psi_host, self._psi_bytes, self._esz, False, "psi_host")
         self._ck(lib().sso_step_host(self._h, _ptr(psi_host), int(nsteps)))
 
     def norm(self, psi, stream=None) -> float:
         out = ctypes.c_double()
+        _check_buffer(psi, self._psi_bytes, self._esz, True, "psi")
         self._ck(lib().sso_norm(self._h, _ptr(psi), ctypes.byref(out), _stream(stream)))
         return out.value
+
+    def profile_step(self, psi, nsteps: int, stream=None):
+        """sso_profile_step: [(pass name, launches, mean microseconds)] for the pass kinds that ran."""
+        _check_buffer(psi, self._psi_bytes, self._esz, True, "psi")
+        cnt = (ctypes.c_int64 * PASS_KINDS)()
+        us = (ctypes.c_double * PASS_KINDS)()
+        self._ck(lib().sso_profile_step(self._h, _ptr(psi), int(nsteps), _stream(stream), cnt, us))
+        return [(lib().sso_pass_name(k).decode(), int(cnt[k]), float(us[k])) for k in range(PASS_KINDS) if cnt[k]]
 
     def launch_count(self, nsteps: int) -> int:
         n = ctypes.c_int64()

@@ -78,25 +78,6 @@ __global__ void build_kphase_kernel(const double *__restrict__ kv, void *__restr
     reinterpret_cast<C *>(out)[i] = h;
 }
 
-// phase of a homogeneous E field along the line axis in the permuted layout:
-// out[slot] = exp(-i (tau/2) (E_na + [full] E_nb)[axis] r(nat(slot)))
-template <typename T>
-__global__ void build_ephase_kernel(void *__restrict__ out, int n, const int *__restrict__ slot_nat, double dx, double half_dt,
-                                    const double *__restrict__ step_avg, long long na, long long nb, int full, int ndim, int axis) {
-    using C = typename Cx2<T>::type;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    double e = step_avg[na * ndim + axis];
-    if (full) e += step_avg[nb * ndim + axis];
-    const double r = ((double)slot_nat[i] - (double)(n / 2)) * dx;
-    double s, c;
-    sincos(-e * half_dt * r, &s, &c);
-    C h;
-    h.x = (T)c;
-    h.y = (T)s;
-    reinterpret_cast<C *>(out)[i] = h;
-}
-
 // homogeneous E field, all passes of one sso_step call at once (2D/3D).  For every lattice axis with a field
 // component, row j of out[ax] (n[ax] complex entries) is the phase exp(-i (tau/2) c_j r) with
 //   j = 0        c = Ebar[n0]                      opening half step        (natural order)
@@ -253,7 +234,6 @@ struct Axis {
     int *d_slot_nat = nullptr;     // device int[n]
     double *d_kv = nullptr;        // device double[n]: k in the layout this axis uses in the kinetic pass
     void *d_kph = nullptr;         // device complex[n]: Schroedinger phase table in the same layout
-    void *d_ephase = nullptr;      // device complex[n]: E-field phase along this axis (last axis only)
 };
 
 }  // namespace sso
@@ -283,7 +263,14 @@ struct sso_plan {
     int vrep = VREP_TABLE;
     bool kph_valid = false;
     int opt_tl_contig = 0, opt_tl_strided = 0, opt_groups = 0, opt_ring = 0, opt_maxt = 0, opt_sring = 0;
-    int dbg_skip = 0;  // development only: bit 0 skip DIF, bit 1 skip DIT, bit 2 skip the pointwise factor (wrong results)
+    int device = 0, num_sms = 0;  // the device the plan was created on, its SM count
+    size_t smem_optin = 0;        // largest dynamic shared memory a CTA may opt in to on that device
+    struct ProfEvent {
+        int kind;
+        cudaEvent_t a, b;
+    };
+    std::vector<ProfEvent> *prof = nullptr;  // non-NULL while sso_profile_step brackets every launch with events
+    bool v_valid = true;          // false between a change of the potential representation and the next sso_set_potential
     double *d_partial = nullptr, *d_norm = nullptr;
     unsigned *d_sched = nullptr;  // tile scheduler of the pass kernel (zero between launches)
     void *d_hostbuf = nullptr;
@@ -314,14 +301,28 @@ template <typename V> static cudaError_t upload(void **dst, const std::vector<V>
     return cudaMemcpy(*dst, src.data(), src.size() * sizeof(V), cudaMemcpyHostToDevice);
 }
 
-// development aid: SSO_DEBUG_SYNC=1 synchronises after every pass and names the one that failed
-static int dbg_sync(sso_plan *plan, cudaStream_t st, const char *what, cudaError_t e) {
-    static int on = -1;
-    if (on < 0) on = getenv("SSO_DEBUG_SYNC") ? 1 : 0;
-    if (e == cudaSuccess && on) e = cudaStreamSynchronize(st);
+static int pass_status(sso_plan *plan, const char *what, cudaError_t e) {
     if (e != cudaSuccess) return cuda_fail(plan, e, what);
     return SSO_OK;
 }
+
+// brackets the launches of one pass with CUDA events while the plan is being profiled (sso_profile_step)
+struct PassTimer {
+    sso_plan *p;
+    cudaStream_t st;
+    long idx = -1;
+    PassTimer(sso_plan *plan, int kind, cudaStream_t stream) : p(plan), st(stream) {
+        if (!p->prof) return;
+        sso_plan::ProfEvent e{kind, nullptr, nullptr};
+        if (cudaEventCreate(&e.a) != cudaSuccess || cudaEventCreate(&e.b) != cudaSuccess) return;
+        cudaEventRecord(e.a, st);
+        p->prof->push_back(e);
+        idx = (long)p->prof->size() - 1;
+    }
+    ~PassTimer() {
+        if (idx >= 0) cudaEventRecord((*p->prof)[(size_t)idx].b, st);
+    }
+};
 
 static bool is_pow2(long long v) { return v > 0 && (v & (v - 1)) == 0; }
 
@@ -379,8 +380,17 @@ int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double
         cudaGetLastError();
         return fail(nullptr, SSO_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
     }
+    int dev = 0, num_sms = 0, optin = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess || num_sms < 1) {
+        cudaGetLastError();
+        return fail(nullptr, SSO_ERR_CUDA, "cannot query the current CUDA device");
+    }
     plan = new (std::nothrow) sso_plan();
     if (!plan) return fail(nullptr, SSO_ERR_ALLOC, "out of host memory");
+    plan->device = dev;
+    plan->num_sms = num_sms;
+    plan->smem_optin = (size_t)optin;
     plan->ndim = ndim;
     plan->ncomp = ncomp;
     plan->precision = precision;
@@ -454,7 +464,6 @@ int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double
         kinetic_layout(plan, a, kv);
         if (e == cudaSuccess) e = upload((void **)&A.d_kv, kv);
         if (e == cudaSuccess) e = cudaMalloc(&A.d_kph, (size_t)n * plan->esize());
-        if (e == cudaSuccess) e = cudaMalloc(&A.d_ephase, (size_t)n * plan->esize());
         if (e != cudaSuccess) {
             int rc = cuda_fail(nullptr, e, "plan tables");
             sso_destroy(plan);
@@ -490,7 +499,6 @@ int sso_destroy(sso_plan *plan) {
         cudaFree(A.d_slot_nat);
         cudaFree(A.d_kv);
         cudaFree(A.d_kph);
-        cudaFree(A.d_ephase);
     }
     cudaFree(plan->d_avg);
     cudaFree(plan->d_vtab);
@@ -536,6 +544,7 @@ int sso_set_potential(sso_plan *plan, const double *V, int on_device, void *stre
     cudaFree(plan->d_vtab);
     cudaFree(plan->d_vfull);
     plan->d_vtab = plan->d_vfull = nullptr;
+    plan->v_valid = false;
     cudaError_t e = cudaMalloc(&plan->d_vtab, entry * total);
     if (e == cudaSuccess && plan->ndim >= 2) e = cudaMalloc(&plan->d_vfull, entry * total);
     if (e != cudaSuccess) {
@@ -555,6 +564,7 @@ int sso_set_potential(sso_plan *plan, const double *V, int on_device, void *stre
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     cudaFree(tmp);
     if (e != cudaSuccess) return cuda_fail(plan, e, "potential table kernel");
+    plan->v_valid = true;
     return SSO_OK;
 }
 
@@ -639,9 +649,6 @@ int sso_set_option(sso_plan *plan, int option, int64_t value) {
             if (value < 0 || value > 512 || (value > 0 && !is_pow2(value))) return fail(plan, SSO_ERR_INVALID, "lines per tile must be 0 or a power of two <= 512");
             (option == SSO_OPT_LINES_PER_TILE_CONTIG ? plan->opt_tl_contig : plan->opt_tl_strided) = (int)value;
             return SSO_OK;
-        case 100:
-            plan->dbg_skip = (int)value;
-            return SSO_OK;
         case SSO_OPT_RING_BUFFERS:
             if (value < 0 || value > 16) return fail(plan, SSO_ERR_INVALID, "ring buffers must be in [0, 16]");
             plan->opt_ring = (int)value;
@@ -662,8 +669,11 @@ int sso_set_option(sso_plan *plan, int option, int64_t value) {
             if (value != VREP_TABLE && value != VREP_ANGLE) return fail(plan, SSO_ERR_INVALID, "potential phase mode must be 0 or 1");
             if ((int)value != plan->vrep) {
                 plan->vrep = (int)value;
-                // the table is rebuilt by the next sso_set_potential; until then V = 0
-                return sso_set_potential(plan, nullptr, 0, nullptr);
+                // the plan does not keep V itself: the tables are re-made empty in the new representation and
+                // sso_step refuses to run until sso_set_potential has been called again
+                const int rc = sso_set_potential(plan, nullptr, 0, nullptr);
+                plan->v_valid = false;
+                return rc;
             }
             return SSO_OK;
     }
@@ -735,14 +745,12 @@ struct PassSpec {
     int pw;        // PW_*
     int sign;      // sign of the DIF transform
     int do_dif, do_dit, unpermute, mid_on, pre_v, post_v;
-    int v_mid_full;
     int nrep;
     long long n;   // step index
 };
 
 int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
-    if ((plan->dbg_skip & 16) && s.axis == 0 && plan->ndim > 1) return SSO_OK;               // development: no kinetic pass
-    if ((plan->dbg_skip & 32) && s.axis == plan->ndim - 1 && plan->ndim > 1) return SSO_OK;  // development: no potential pass
+    PassTimer timer(plan, plan->ndim == 1 ? SSO_PASS_LINE_1D : (s.axis == 0 ? SSO_PASS_KINETIC : (s.do_dif ? SSO_PASS_MIDDLE_FORWARD : SSO_PASS_MIDDLE_INVERSE)), st);
     const Geometry g = geometry(plan, s.axis);
     const Axis &A = plan->ax[s.axis];
     const int cc = s.pw == PW_KD2 ? 2 : (s.pw == PW_KD4 ? 4 : 1);
@@ -767,19 +775,15 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
     a.rest1 = g.rest1;
     a.oaxA = g.oaxA;
     a.oaxB = g.oaxB;
-    a.do_dif = (plan->dbg_skip & 1) ? 0 : s.do_dif;
-    a.do_dit = (plan->dbg_skip & 2) ? 0 : s.do_dit;
+    a.do_dif = s.do_dif;
+    a.do_dit = s.do_dit;
     a.unpermute = s.unpermute;
-    a.mid_on = (plan->dbg_skip & 4) ? 0 : s.mid_on;
-    a.dbg_copy = (plan->dbg_skip & 8) ? 1 : 0;
-    a.dbg_flags = (plan->dbg_skip >> 6) & 3;
+    a.mid_on = s.mid_on;
     a.pre_v = s.pre_v;
     a.post_v = s.post_v;
     a.nrep = s.nrep;
     a.vtab = plan->d_vtab;
     a.vrep = plan->vrep;
-    a.v_mid_full = s.v_mid_full;
-    a.ephase = nullptr;
     a.step_avg = plan->d_avg;
     a.field_kind = plan->field_kind;
     a.ndim = plan->ndim;
@@ -803,16 +807,6 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
         a.kv0 = A.d_kv;
         a.kv1 = g.oaxA >= 0 ? plan->ax[g.oaxA].d_kv : nullptr;
         a.kv2 = g.oaxB >= 0 ? plan->ax[g.oaxB].d_kv : nullptr;
-    } else if (s.pw == PW_V && s.mid_on && plan->field_kind == SSO_FIELD_E && plan->e_along_last) {
-        // phase of the field component along the line, rebuilt for this step (prep kernel)
-        const int blocks = (A.n + 127) / 128;
-        if (plan->precision == SSO_C128)
-            build_ephase_kernel<double><<<blocks, 128, 0, st>>>(A.d_ephase, A.n, A.d_slot_nat, A.dx, 0.5 * plan->dt, plan->d_avg, s.n, s.n + 1, s.v_mid_full, plan->ndim, s.axis);
-        else
-            build_ephase_kernel<float><<<blocks, 128, 0, st>>>(A.d_ephase, A.n, A.d_slot_nat, A.dx, 0.5 * plan->dt, plan->d_avg, s.n, s.n + 1, s.v_mid_full, plan->ndim, s.axis);
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return cuda_fail(plan, e, "ephase kernel");
-        a.ephase = A.d_ephase;
     }
     LaunchFn fn = find_launch(plan->precision, A.n, g.strided ? 1 : 0, s.pw, s.sign);
     if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no kernel built for this pass");
@@ -831,10 +825,10 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
     if (GT % 32 == 0) {
         const int maxthreads = 512;
         G = plan->opt_groups > 0 ? plan->opt_groups : maxthreads / GT;
-        while (G > 1 && ((size_t)G * greg + twbytes > 227 * 1024 - 1024 || G * GT > maxthreads)) --G;
+        while (G > 1 && ((size_t)G * greg + twbytes > (size_t)plan->smem_optin - 1024 || G * GT > maxthreads)) --G;
         if (G > 15) G = 15;
         if (G < 1) G = 1;
-        const long long tiles_per_sm = (work + 147) / 148;
+        const long long tiles_per_sm = (work + plan->num_sms - 1) / plan->num_sms;
         if (G > tiles_per_sm) G = (int)(tiles_per_sm > 0 ? tiles_per_sm : 1);
     }
     a.G = G;
@@ -842,9 +836,8 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
     a.gstride = (int)(greg / esz);
     const unsigned threads = (unsigned)(G * GT);
     size_t smem = twbytes + (size_t)G * greg;
-    if ((plan->dbg_skip >> 8) & 1) smem = smem < 120 * 1024 ? 120 * 1024 : smem;  // development: one CTA per SM
     cudaError_t e = fn(a, threads, smem, st);
-    return dbg_sync(plan, st, g.strided ? "direct strided pass" : "direct contiguous pass", e);
+    return pass_status(plan, g.strided ? "direct strided pass" : "direct contiguous pass", e);
 }
 
 
@@ -877,7 +870,7 @@ void choose_groups(const sso_plan *plan, int GT, int bmax, long long tiles_per_c
 // contiguous-axis pass of a 2D/3D lattice through the ring pipeline (sso_ring.cuh).  `row` selects the field
 // phase row of this call (build_erows_kernel): 0 opening, j merged after step j-1, nsteps closing.
 int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStream_t st) {
-    if (plan->dbg_skip & 32) return SSO_OK;  // development: no potential pass
+    PassTimer timer(plan, mode == MODE_OPEN ? SSO_PASS_OPENING : (mode == MODE_MID ? SSO_PASS_POTENTIAL : SSO_PASS_CLOSING), st);
     const int last = plan->ndim - 1;
     const Axis &A = plan->ax[last];
     const int U = A.n / 16;
@@ -894,11 +887,11 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     const long long ntiles = lines * plan->ncomp / TL;
     if (ntiles > 0x7fffffffLL) return fail(plan, SSO_ERR_UNSUPPORTED, "too many tiles");
     // G groups, each with its own NBG buffers (NBG = 2: the next tile loads while the current one is worked on)
-    const size_t avail = 227 * 1024 - 256 - twbytes;
+    const size_t avail = (size_t)plan->smem_optin - 256 - twbytes;
     const int bmax = (int)(avail / bufbytes);
     if (bmax < 1) return fail(plan, SSO_ERR_UNSUPPORTED, "line too long for the ring pipeline");
     int G = 1, NBG = 1;
-    choose_groups(plan, GT, bmax, (ntiles + 147) / 148, &G, &NBG);
+    choose_groups(plan, GT, bmax, (ntiles + plan->num_sms - 1) / plan->num_sms, &G, &NBG);
     const int maxt = plan->opt_maxt ? plan->opt_maxt : (G * GT <= 384 ? 384 : 512);
     const int NB = G * NBG;
     RingArgs a{};
@@ -918,7 +911,6 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     a.rest1 = g.rest1;
     a.vtab = mode == MODE_MID ? plan->d_vfull : plan->d_vtab;
     a.vrep = plan->vrep;
-    a.dbg_nophase = (plan->dbg_skip & 4) ? 1 : 0;
     if (plan->field_kind == SSO_FIELD_E) {
         if (plan->e_axis_on[last]) a.eline = (const char *)plan->d_erow[last] + (size_t)row * A.n * esz;
         if (g.oaxA >= 0 && plan->e_axis_on[g.oaxA]) a.eoA = (const char *)plan->d_erow[g.oaxA] + (size_t)row * plan->ax[g.oaxA].n * esz;
@@ -927,9 +919,9 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     RingLaunchFn fn = find_ring(plan->precision, A.n, mode, maxt);
     if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no ring kernel built for this line length");
     const size_t smem = twbytes + (size_t)NB * bufbytes + (size_t)NB * 8 + (size_t)(NB + 1) * 4;
-    const unsigned grid = (unsigned)(ntiles < 148 ? ntiles : 148);
+    const unsigned grid = (unsigned)(ntiles < plan->num_sms ? ntiles : plan->num_sms);
     cudaError_t e = fn(a, (unsigned)(G * GT), smem, grid, st);
-    return dbg_sync(plan, st, mode == MODE_OPEN ? "ring opening pass" : (mode == MODE_MID ? "ring potential pass" : "ring closing pass"), e);
+    return pass_status(plan, mode == MODE_OPEN ? "ring opening pass" : (mode == MODE_MID ? "ring potential pass" : "ring closing pass"), e);
 }
 
 
@@ -937,17 +929,15 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
                                   const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn encode_tiled_fn() {
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
+    // a driver entry point is process-wide; the initialiser of a function-local static runs once, thread-safely
+    static const EncodeTiledFn fn = [] {
         void *p = nullptr;
         cudaDriverEntryPointQueryResult q;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)p;
-        else
-            cudaGetLastError();
-    }
+            return (EncodeTiledFn)p;
+        cudaGetLastError();
+        return (EncodeTiledFn) nullptr;
+    }();
     return fn;
 }
 
@@ -972,8 +962,8 @@ SRingShape sring_shape(const sso_plan *plan, int axis, int cc) {
         const int pitch = A.n + A.n / 16 + (Gn / TL > 1 ? Gn / TL : 1);
         const size_t bb = ((size_t)cc * TL * pitch * esz + 127) & ~(size_t)127;
         const size_t tw = (size_t)twiddle_count_padded(A.n) * esz;
-        if (bb + tw > 227 * 1024 - 256) return false;
-        *bmax_out = (int)((227 * 1024 - 256 - tw) / bb);
+        if (bb + tw > (size_t)plan->smem_optin - 256) return false;
+        *bmax_out = (int)(((size_t)plan->smem_optin - 256 - tw) / bb);
         return true;
     };
     int TL = 0, bm = 0;
@@ -991,12 +981,12 @@ SRingShape sring_shape(const sso_plan *plan, int axis, int cc) {
     r.pitch = A.n + A.n / 16 + (Gn / TL > 1 ? Gn / TL : 1);
     r.bufbytes = ((size_t)cc * TL * r.pitch * esz + 127) & ~(size_t)127;
     r.twbytes = (size_t)twiddle_count_padded(A.n) * esz;
-    const int bmax = (int)((227 * 1024 - 256 - r.twbytes) / r.bufbytes);
+    const int bmax = (int)(((size_t)plan->smem_optin - 256 - r.twbytes) / r.bufbytes);
     if (bmax < 1) return r;
     int NBG = 1;
     const long long outer = plan->npts / (A.n * g.inner);
     const long long ntiles = (cc == 1 ? outer * plan->ncomp : 1) * (g.inner / TL);
-    choose_groups(plan, r.GT, bmax, (ntiles + 147) / 148, &r.G, &NBG);
+    choose_groups(plan, r.GT, bmax, (ntiles + plan->num_sms - 1) / plan->num_sms, &r.G, &NBG);
     r.NB = r.G * NBG;
     r.box_rows = A.n < 256 ? A.n : 256;
     r.ok = true;
@@ -1004,7 +994,7 @@ SRingShape sring_shape(const sso_plan *plan, int axis, int cc) {
 }
 
 int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long n, const SRingShape &sh, cudaStream_t st) {
-    if ((plan->dbg_skip & 16) && axis == 0) return SSO_OK;  // development: no kinetic pass
+    PassTimer timer(plan, smode == SMODE_DIF ? SSO_PASS_MIDDLE_FORWARD : (smode == SMODE_DIT ? SSO_PASS_MIDDLE_INVERSE : SSO_PASS_KINETIC), st);
     const Axis &A = plan->ax[axis];
     const Geometry g = geometry(plan, axis);
     const int esz = (int)plan->esize();
@@ -1027,7 +1017,6 @@ int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long 
     a.psi = psi;
     a.inner = g.inner;
     a.comp_stride = plan->npts;
-    a.direct_store = (plan->dbg_skip & 512) ? 0 : 1;  // measured faster than the TMA store for every row width, 32 bytes included
     a.tw = A.tw;
     a.TL = sh.TL;
     a.pitch = sh.pitch;
@@ -1061,9 +1050,9 @@ int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long 
     SRingLaunchFn fn = find_sring(plan->precision, A.n, smode);
     if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no strided ring kernel built for this line length");
     const size_t smem = sh.twbytes + (size_t)sh.NB * sh.bufbytes + (size_t)sh.NB * 8 + (size_t)(sh.NB + 1) * 4;
-    const unsigned grid = (unsigned)(ntiles < 148 ? ntiles : 148);
+    const unsigned grid = (unsigned)(ntiles < plan->num_sms ? ntiles : plan->num_sms);
     cudaError_t e = fn(a, &plan->tmap[axis], (unsigned)(a.G * sh.GT), smem, grid, st);
-    return dbg_sync(plan, st, smode == SMODE_DIF ? "strided ring DIF pass" : (smode == SMODE_DIT ? "strided ring DIT pass" : "strided ring kinetic pass"), e);
+    return pass_status(plan, smode == SMODE_DIF ? "strided ring DIF pass" : (smode == SMODE_DIT ? "strided ring DIT pass" : "strided ring kinetic pass"), e);
 }
 
 // field phase rows for steps [n0, n0 + ns) of a 2D/3D call
@@ -1081,6 +1070,7 @@ int build_erows(sso_plan *plan, long long n0, long long ns, cudaStream_t st) {
         any = true;
     }
     if (!any) return SSO_OK;
+    PassTimer timer(plan, SSO_PASS_TABLES, st);
     e.slot_nat_last = plan->ax[plan->ndim - 1].d_slot_nat;
     e.step_avg = plan->d_avg;
     e.n0 = n0;
@@ -1109,6 +1099,7 @@ long long erow_chunk(const sso_plan *p) {
 int build_kphase(sso_plan *plan, long long n, cudaStream_t st) {
     const bool shifted = plan->field_kind == SSO_FIELD_A;
     if (plan->kph_valid && !shifted) return SSO_OK;
+    PassTimer timer(plan, SSO_PASS_TABLES, st);
     for (int a = 0; a < plan->ndim; ++a) {
         Axis &A = plan->ax[a];
         const double scale = a == 0 ? 1.0 / (double)plan->npts : 1.0;
@@ -1165,6 +1156,8 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
     if (nsteps == 0) return SSO_OK;
     if (plan->field_kind != SSO_FIELD_NONE && plan->tindex + nsteps > plan->nvals)
         return fail(plan, SSO_ERR_STATE, "field table shorter than the steps requested");
+    if (!plan->v_valid || !plan->d_vtab || (plan->ndim >= 2 && !plan->d_vfull))
+        return fail(plan, SSO_ERR_STATE, "no potential table: call sso_set_potential (again) before sso_step");
     cudaStream_t st = (cudaStream_t)stream;
     const int nd = plan->ndim;
     const int kpw = kinetic_pw(plan);
@@ -1176,7 +1169,7 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
         const long long chunk = kshift ? 1 : nsteps;  // step-dependent kinetic tables force one launch per step
         for (long long s = 0; s < nsteps; s += chunk) {
             if (plan->ncomp == 1 && (rc = build_kphase(plan, n0 + s, st)) != SSO_OK) return rc;
-            PassSpec ps{0, kpw, -1, 1, 1, 0, 1, 1, 1, 0, (int)chunk, n0 + s};
+            PassSpec ps{0, kpw, -1, 1, 1, 0, 1, 1, 1, (int)chunk, n0 + s};
             if (chunk > 0x7fffffffLL) return fail(plan, SSO_ERR_INVALID, "nsteps too large");
             if ((rc = launch(plan, psi, ps, st)) != SSO_OK) return rc;
         }
@@ -1199,21 +1192,21 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
                 if (nd == 3) {  // F_1, stored in network order
                     if (shm.ok) rc = launch_sring_pass(plan, psi, 1, SMODE_DIF, n, shm, st);
                     else {
-                        PassSpec mid{1, PW_NONE, -1, 1, 0, 0, 0, 0, 0, 0, 1, n};
+                        PassSpec mid{1, PW_NONE, -1, 1, 0, 0, 0, 0, 0, 1, n};
                         rc = launch(plan, psi, mid, st);
                     }
                     if (rc != SSO_OK) return rc;
                 }
                 if (shk.ok) rc = launch_sring_pass(plan, psi, 0, kpw == PW_KS ? SMODE_KS : (kpw == PW_KD2 ? SMODE_KD2 : SMODE_KD4), n, shk, st);
                 else {
-                    PassSpec kin{0, kpw, -1, 1, 1, 0, 1, 0, 0, 0, 1, n};  // F_0 K F_0^-1
+                    PassSpec kin{0, kpw, -1, 1, 1, 0, 1, 0, 0, 1, n};  // F_0 K F_0^-1
                     rc = launch(plan, psi, kin, st);
                 }
                 if (rc != SSO_OK) return rc;
                 if (nd == 3) {  // F_1^-1 from network order
                     if (shm.ok) rc = launch_sring_pass(plan, psi, 1, SMODE_DIT, n, shm, st);
                     else {
-                        PassSpec mid{1, PW_NONE, -1, 0, 1, 0, 0, 0, 0, 0, 1, n};
+                        PassSpec mid{1, PW_NONE, -1, 0, 1, 0, 0, 0, 0, 1, n};
                         rc = launch(plan, psi, mid, st);
                     }
                     if (rc != SSO_OK) return rc;
@@ -1225,6 +1218,48 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
     }
     plan->tindex += nsteps;
     return SSO_OK;
+}
+
+int sso_profile_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream, int64_t *count, double *mean_us) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (!count || !mean_us) return fail(plan, SSO_ERR_INVALID, "count or mean_us is NULL");
+    for (int k = 0; k < SSO_PASS_KINDS; ++k) {
+        count[k] = 0;
+        mean_us[k] = 0.0;
+    }
+    std::vector<sso_plan::ProfEvent> ev;
+    plan->prof = &ev;
+    int rc = sso_step(plan, psi, nsteps, stream);
+    plan->prof = nullptr;
+    cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+    for (auto &p : ev) {
+        float ms = 0.f;
+        if (rc == SSO_OK && e == cudaSuccess && cudaEventElapsedTime(&ms, p.a, p.b) == cudaSuccess && p.kind >= 0 && p.kind < SSO_PASS_KINDS) {
+            count[p.kind] += 1;
+            mean_us[p.kind] += (double)ms * 1e3;
+        }
+        cudaEventDestroy(p.a);
+        cudaEventDestroy(p.b);
+    }
+    for (int k = 0; k < SSO_PASS_KINDS; ++k)
+        if (count[k] > 0) mean_us[k] /= (double)count[k];
+    if (rc != SSO_OK) return rc;
+    if (e != cudaSuccess) return cuda_fail(plan, e, "sso_profile_step");
+    return SSO_OK;
+}
+
+const char *sso_pass_name(int kind) {
+    switch (kind) {
+        case SSO_PASS_OPENING: return "opening [V/2 . F_last]";
+        case SSO_PASS_POTENTIAL: return "potential [F_last^-1 . V . F_last]";
+        case SSO_PASS_CLOSING: return "closing [F_last^-1 . V/2]";
+        case SSO_PASS_KINETIC: return "kinetic [F_0 . K . F_0^-1]";
+        case SSO_PASS_MIDDLE_FORWARD: return "middle axis [F_1]";
+        case SSO_PASS_MIDDLE_INVERSE: return "middle axis [F_1^-1]";
+        case SSO_PASS_LINE_1D: return "1D line, all steps in one launch";
+        case SSO_PASS_TABLES: return "per-step tables";
+    }
+    return "";
 }
 
 int sso_step_host(sso_plan *plan, void *psi_host, int64_t nsteps) {

@@ -6,7 +6,7 @@
 
 namespace sso {
 
-enum : int { PW_NONE = 0, PW_V = 1, PW_KS = 2, PW_KD2 = 3, PW_KD4 = 4 };
+enum : int { PW_NONE = 0, PW_KS = 2, PW_KD2 = 3, PW_KD4 = 4 };
 
 // V-phase representation
 enum : int { VREP_TABLE = 0, VREP_ANGLE = 1 };
@@ -29,16 +29,12 @@ struct PassArgs {
     int oaxA, oaxB;          // lattice axes that ia and ib run along (-1: absent)
     // structure of the pass
     int do_dif, do_dit, unpermute;
-    int dbg_flags;           // development only: bit 0 no table prefetch, bit 1 no next-tile prefetch
-    int dbg_copy;            // development only: load and store in the coalesced layout, nothing in between
     int mid_on;              // apply the pointwise factor between DIF and DIT
     int pre_v, post_v;       // 0 none; 1 natural-order table (1D); 2 gather from the permuted table (opening pass)
     int nrep;                // repetitions inside the kernel (1D persistent stepping), >= 1
     // potential phase
-    const void *vtab;        // complex h = exp(-i V tau/2) (VREP_TABLE) or real angle -V tau/2 (VREP_ANGLE)
+    const void *vtab;        // 1D: complex h = exp(-i V tau/2) (VREP_TABLE) or real angle -V tau/2 (VREP_ANGLE), natural order
     int vrep;
-    int v_mid_full;          // mid factor is the full (merged) phase h^2
-    const void *ephase;      // complex[N] extra phase along the line (permuted layout) or NULL
     // field table
     const double *step_avg;  // device [nvals][ndim] or NULL
     int field_kind;          // SSO_FIELD_*
@@ -92,7 +88,6 @@ struct RingArgs {
     int vrep;                 // VREP_TABLE (complex phases) or VREP_ANGLE (real angles, sincos in the kernel)
     const void *eline;        // complex[N] field phase along the line for this pass (same order as vtab) or NULL
     const void *eoA, *eoB;    // complex field phase rows of the other axes, indexed by ia / ib, or NULL
-    int dbg_nophase;          // development only: skip the pointwise factor (wrong results)
 };
 
 using RingLaunchFn = cudaError_t (*)(const RingArgs &, unsigned threads, size_t smem, unsigned grid, cudaStream_t st);
@@ -103,7 +98,6 @@ struct SRingArgs {
     void *psi;                // device base of psi (stores from registers; loads go through the tensor map)
     long long inner;          // element stride along the line
     long long comp_stride;    // elements between components
-    int direct_store;         // results are stored from registers (default) instead of through the buffer with a TMA store
     const void *tw;           // twiddle blocks of the line axis
     int ntiles;               // tiles of TL adjacent lines (x all components when they are independent)
     int TL;                   // adjacent lines per tile: one row of a tile is TL complex numbers, contiguous in memory

@@ -2,6 +2,8 @@
 // Compiled once per pair with -DSSO_T=<float|double> -DSSO_TNAME=<f32|f64> -DSSO_N=<n>
 // (see paper_1012_3911_b200/build.py); each object exports one lookup function that the
 // dispatcher in sso_api.cu calls.
+#include <atomic>
+
 #include "sso_pass.cuh"
 #include "sso_ring.cuh"
 #include "sso_sring.cuh"
@@ -13,36 +15,38 @@
 
 namespace sso {
 
+// cudaFuncSetAttribute is per device: opt a kernel in to large dynamic shared memory once per device (bit d of
+// `done` = device d; devices beyond 63 repeat the call, which is harmless)
+template <typename K> static cudaError_t opt_in_smem(K kern, std::atomic<unsigned long long> &done, int *dev_out = nullptr, int *sms_out = nullptr) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev_out) *dev_out = dev;
+    const unsigned long long bit = dev < 64 ? 1ull << dev : 0ull;
+    if (!(done.load(std::memory_order_acquire) & bit) || sms_out) {
+        int optin = 0, sms = 0;
+        if ((e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev)) != cudaSuccess) return e;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        if (sms_out) *sms_out = sms;
+        if (!(done.load(std::memory_order_acquire) & bit)) {
+            if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)) != cudaSuccess) return e;
+            done.fetch_or(bit, std::memory_order_release);
+        }
+    }
+    return cudaSuccess;
+}
+
 template <typename T, int N, bool STRIDED, int PW, int SIGN>
 cudaError_t launch_pass(const PassArgs &a, unsigned threads, size_t smem, cudaStream_t st) {
     auto kern = pass_kernel<T, N, STRIDED, PW, SIGN>;
-    static bool attr_done = false;
-    static int num_sms = 0;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
-        int dev = 0;
-        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
-        if ((e = cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-        attr_done = true;
-    }
-    // resident CTAs per SM for this block shape (cached: a plan uses one or two shapes per kernel)
-    static unsigned key_threads[4] = {0, 0, 0, 0};
-    static size_t key_smem[4] = {0, 0, 0, 0};
-    static int key_occ[4] = {0, 0, 0, 0};
-    static int key_n = 0;
+    static std::atomic<unsigned long long> done{0};
+    int dev = 0, num_sms = 0;
+    cudaError_t e = opt_in_smem(kern, done, &dev, &num_sms);
+    if (e != cudaSuccess) return e;
+    // one wave of persistent CTAs: resident CTAs per SM for this block shape x SM count of the current device
     int occ = 0;
-    for (int i = 0; i < key_n; ++i)
-        if (key_threads[i] == threads && key_smem[i] == smem) occ = key_occ[i];
-    if (occ == 0) {
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (int)threads, smem);
-        if (e != cudaSuccess) return e;
-        if (occ < 1) return cudaErrorLaunchOutOfResources;
-        const int slot = key_n < 4 ? key_n++ : 3;
-        key_threads[slot] = threads;
-        key_smem[slot] = smem;
-        key_occ[slot] = occ;
-    }
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (int)threads, smem)) != cudaSuccess) return e;
+    if (occ < 1) return cudaErrorLaunchOutOfResources;
     long long grid = (long long)occ * num_sms;
     const long long need = ((long long)a.ntiles + a.G - 1) / a.G;
     if (grid > need) grid = need;
@@ -70,12 +74,9 @@ static cudaError_t launch_pdl(K kern, unsigned grid, unsigned threads, size_t sm
 template <typename T, int N, int MODE, int SIGN, int MAXT>
 cudaError_t launch_ring(const RingArgs &a, unsigned threads, size_t smem, unsigned grid, cudaStream_t st) {
     auto kern = ring_kernel<T, N, MODE, SIGN, MAXT>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    static std::atomic<unsigned long long> done{0};
+    cudaError_t e = opt_in_smem(kern, done);
+    if (e != cudaSuccess) return e;
     if (threads > (unsigned)MAXT) return cudaErrorInvalidConfiguration;
     return launch_pdl(kern, grid, threads, smem, st, a);
 }
@@ -83,12 +84,9 @@ cudaError_t launch_ring(const RingArgs &a, unsigned threads, size_t smem, unsign
 template <typename T, int N, int SMODE>
 cudaError_t launch_sring(const SRingArgs &a, const void *tensor_map, unsigned threads, size_t smem, unsigned grid, cudaStream_t st) {
     auto kern = sring_kernel<T, N, SMODE>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    static std::atomic<unsigned long long> done{0};
+    cudaError_t e = opt_in_smem(kern, done);
+    if (e != cudaSuccess) return e;
     if (threads > 512u) return cudaErrorInvalidConfiguration;
     return launch_pdl(kern, grid, threads, smem, st, a, *reinterpret_cast<const CUtensorMap *>(tensor_map));
 }
@@ -140,8 +138,6 @@ LaunchFn SSO_CAT3(sso_lookup_, SSO_TNAME, SSO_N)(int strided, int pw, int sign) 
     using T = SSO_T;
     constexpr int N = SSO_N;
     if (!strided) {
-        if (pw == PW_V && sign > 0) return &launch_pass<T, N, false, PW_V, +1>;      // potential sandwich, closing pass
-        if (pw == PW_NONE && sign < 0) return &launch_pass<T, N, false, PW_NONE, -1>;  // opening pass
         if (pw == PW_KS && sign < 0) return &launch_pass<T, N, false, PW_KS, -1>;     // 1D step
         if (pw == PW_KD2 && sign < 0) return &launch_pass<T, N, false, PW_KD2, -1>;
         if (pw == PW_KD4 && sign < 0) return &launch_pass<T, N, false, PW_KD4, -1>;

@@ -462,20 +462,13 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
         }
 
         C x[16];
-        if (a.do_dif || a.dbg_copy) {
+        if (a.do_dif) {
 #pragma unroll
             for (int q = 0; q < 16; ++q) x[q] = ld_stream(&gp[(long long)(u + q * U) * estep]);
         } else {
 #pragma unroll
             for (int q = 0; q < 16; ++q) x[q] = ld_stream(&gp[(long long)(u * 16 + q) * estep]);
         }
-        if constexpr (PW == PW_V) {
-            if (a.mid_on && u == 0 && !(a.dbg_flags & 1)) {
-                const size_t esz = a.vrep == VREP_TABLE ? sizeof(C) : sizeof(double);
-                prefetch_l2_bulk(reinterpret_cast<const char *>(a.vtab) + (size_t)line * N * esz, (unsigned)(N * esz));
-            }
-        }
-
         // angle of the homogeneous-field phase contributed by the non-line axes of this line:
         // (tau/2) sum_ax (Ebar_na + [full] Ebar_nb)[ax] * r_ax      (eq. 11, reading G12)
         auto other_axes_angle = [&](long long n_a, long long n_b, bool full) -> double {
@@ -528,7 +521,7 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
         // every thread learns the next tile and asks L2 for its share of that tile
         gsync(gb);  // also orders the twiddle copy (first tile) and lsc before their use
         const int ntile = snext[parity];
-        if (ntile < a.ntiles && !(a.dbg_flags & 2)) {
+        if (ntile < a.ntiles) {
             long long tile2 = CC == 1 ? ntile / a.ncomp : ntile;
             const int comp2 = CC == 1 ? ntile % a.ncomp : c;
             const long long line2 = tile2 * TL + t;
@@ -561,27 +554,7 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
             if (a.do_dif) DifChain<T, N, 0, SIGN>::run(x, u, stw, sl, gb);
 
             if (a.mid_on) {
-                if constexpr (PW == PW_V) {
-                    // merged or half potential phase in the permuted order: register q of thread u is
-                    // table slot q U + u (coalesced across u)
-                    if (a.field_kind == 1 && u == 0) lsc[t] = expi<T>(-other_axes_angle(n, n + 1, a.v_mid_full != 0));
-                    if (a.field_kind == 1) gsync(gb);
-                    const long long vb = line * (long long)N + u;
-#pragma unroll
-                    for (int q = 0; q < 16; ++q) {
-                        C h;
-                        if (a.vrep == VREP_TABLE) {
-                            h = reinterpret_cast<const C *>(a.vtab)[vb + q * U];
-                            if (a.v_mid_full) h = cmul(h, h);
-                        } else {
-                            const double ang = reinterpret_cast<const double *>(a.vtab)[vb + q * U];
-                            h = expi<T>(a.v_mid_full ? 2.0 * ang : ang);
-                        }
-                        if (a.field_kind == 1) h = cmul(h, lsc[t]);
-                        if (a.ephase) h = cmul(h, reinterpret_cast<const C *>(a.ephase)[q * U + u]);
-                        x[q] = cmul(x[q], h);
-                    }
-                } else if constexpr (PW == PW_KS) {
+                if constexpr (PW == PW_KS) {
                     const bool has_lsc = a.kph1 || a.kph2;
                     const C *__restrict__ k0 = reinterpret_cast<const C *>(a.kph0);
 #pragma unroll
@@ -626,7 +599,7 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
 #pragma unroll
             for (int q = 0; q < 16; ++q) x[q] = rb[lin_delta(q, U)];
         }
-        if (a.do_dit || a.unpermute || a.dbg_copy) {
+        if (a.do_dit || a.unpermute) {
 #pragma unroll
             for (int q = 0; q < 16; ++q) st_stream(&gp[(long long)(u + q * U) * estep], x[q]);
         } else {

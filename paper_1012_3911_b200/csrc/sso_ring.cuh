@@ -16,8 +16,6 @@
 // instruction).  The pass is launched with programmatic dependent launch: its setup overlaps the drain of the
 // previous pass of the stream, and it waits (griddepcontrol.wait) before it touches psi.
 #pragma once
-#include <cstdio>
-
 #include "sso_pass.cuh"
 
 namespace sso {
@@ -87,23 +85,6 @@ __device__ __forceinline__ void prefetch_l2_bulk_plain(const void *p, unsigned b
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
-#ifdef SSO_TIMELINE
-#define SSO_TL_DECL long long tl_[12]; int tli_ = 0;
-#define SSO_TL_MARK do { if (tli_ < 12) tl_[tli_++] = clock64(); } while (0)
-#define SSO_TL_DUMP(tag, blk, grp, j)                                                                              \
-    do {                                                                                                           \
-        if (((blk) == 0 || (blk) == 100) && tid == 0 && grp == 1) {                                                       \
-            printf("%s blk %d tile %d (start %lld):", tag, (int)(blk), j, tl_[0] - t_entry_);                                                             \
-            for (int i_ = 1; i_ < tli_; ++i_) printf(" %lld", tl_[i_] - tl_[i_ - 1]);                              \
-            printf("  total %lld\n", tl_[tli_ - 1] - tl_[0]);                                                      \
-        }                                                                                                          \
-    } while (0)
-#else
-#define SSO_TL_DECL
-#define SSO_TL_MARK
-#define SSO_TL_DUMP(tag, blk, grp, j)
-#endif
-
 template <typename T, int N, int MODE, int SIGN, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     using C = typename CxOf<T>::type;
@@ -120,9 +101,6 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     // claim tiles as they finish, so a CTA's tiles are shared evenly even when their count is no multiple of G
     volatile int *ktile = reinterpret_cast<volatile int *>(full + a.NB);
 
-#ifdef SSO_TIMELINE
-    const long long t_entry_ = clock64();
-#endif
     const int TL = a.TL, GT = a.GT, G = a.G, NB = a.NB;
     const int grp = threadIdx.x / GT;
     const int tid = threadIdx.x - grp * GT;
@@ -257,24 +235,16 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
                 }
             }
         };
-
-        SSO_TL_DECL
-        SSO_TL_MARK;
-        SSO_TL_MARK;
         C x[16];
 #pragma unroll
         for (int q = 0; q < 16; ++q) x[q] = dense[q * U];
-        gsync(gb);
-        SSO_TL_MARK;  // the exchange layout overlaps the bulk-copy layout of other warps' lines
+        gsync(gb);  // the exchange layout overlaps the bulk-copy layout of other warps' lines
 
         if constexpr (MODE == MODE_OPEN) phase(x);
         DifChain<T, N, 0, SIGN>::run(x, u, stw, sl, gb);
-        SSO_TL_MARK;
         if constexpr (MODE == MODE_MID) {
-            if (!a.dbg_nophase) phase(x);
-            SSO_TL_MARK;
+            phase(x);
             DitChain<T, N, LAST, -SIGN>::run(x, u, stw, sl, gb);
-            SSO_TL_MARK;
         } else {
             // registers hold frequency revB[u] + U q at network position 16 u + q: scatter to natural order
             C *wa = sl + padp(a.revB[u]);
@@ -288,8 +258,10 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
             if constexpr (MODE == MODE_CLOSE) phase(x);
         }
 
+        // the buffer was written with ordinary (generic-proxy) stores and is refilled by the bulk-copy engine (async
+        // proxy): every thread orders its accesses before the refill, then the group meets
+        fence_async_smem();
         gsync(gb);  // every thread of the group is done with the buffer: it can take its next tile right away
-        SSO_TL_MARK;
         if (tid == 0) refill(atomicAdd(const_cast<int *>(&ktile[NB]), 1), b);
         // results go straight from registers to global memory (512 contiguous bytes per warp instruction):
         // no second trip through shared memory and nothing to wait for before the buffer is refilled
@@ -298,15 +270,7 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
 #pragma unroll
             for (int q = 0; q < 16; ++q) st_stream(gout + q * U, x[q]);
         }
-        SSO_TL_MARK;
-        SSO_TL_DUMP("ring", blockIdx.x, grp, j);
     }
-#ifdef SSO_TIMELINE
-    const long long t_loop_end_ = clock64();
-#endif
-#ifdef SSO_TIMELINE
-    if ((blockIdx.x == 0 || blockIdx.x == 100) && tid == 0) printf("ring blk %d grp %d: entry->loop end %lld, ->exit %lld\n", (int)blockIdx.x, grp, t_loop_end_ - t_entry_, clock64() - t_entry_);
-#endif
 }
 
 template <typename T, int N, int MODE, int SIGN, int MAXT>

@@ -22,11 +22,6 @@ __device__ __forceinline__ void tma_load_3d(void *smem_dst, const CUtensorMap *m
                  "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
                  : "memory");
 }
-__device__ __forceinline__ void tma_store_3d(const CUtensorMap *map, int c0, int c1, int c2, const void *smem_src) {
-    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2),
-                 "r"(smem_u32(smem_src))
-                 : "memory");
-}
 
 template <typename T, int N, int SMODE>
 __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const __grid_constant__ CUtensorMap tmap) {
@@ -150,8 +145,9 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
 
         if constexpr (SMODE != SMODE_DIF) DitChain<T, N, LAST, +1>::run(x, u, stw, sl, gb);
 
+        fence_async_smem();  // generic-proxy accesses of the buffer before its refill through the async proxy
         gsync(gb);  // every thread of the group is done with the exchange layout
-        if (a.direct_store) {
+        {
             // store from registers (a warp instruction writes 32/TL rows of TL complex numbers) and refill the
             // buffer at once
             if (tid == 0) refill(atomicAdd(const_cast<int *>(&ktile[NB]), 1), b);
@@ -165,29 +161,8 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
 #pragma unroll
                 for (int q = 0; q < 16; ++q) st_stream(gout + (long long)(u + q * U) * a.inner, x[q]);
             }
-        } else {
-            if constexpr (SMODE == SMODE_DIF) {
-#pragma unroll
-                for (int q = 0; q < 16; ++q) dense[(u * 16 + q) * TL] = x[q];
-            } else {
-#pragma unroll
-                for (int q = 0; q < 16; ++q) dense[(u + q * U) * TL] = x[q];
-            }
-            fence_async_smem();
-            gsync(gb);
-            if (tid == 0) {
-                const int o = tile / a.tiles_per_outer, i0 = (tile % a.tiles_per_outer) * TL;
-                for (int cc = 0; cc < CC; ++cc)
-                    for (int j = 0; j < nbox; ++j)
-                        tma_store_3d(&tmap, 2 * i0, j * a.box_rows, CC > 1 ? cc : o, buf + (size_t)(cc * N + j * a.box_rows) * TL);
-                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-                const int kn = atomicAdd(const_cast<int *>(&ktile[NB]), 1);
-                if (kn < nloc) bulk_wait_read();
-                refill(kn, b);
-            }
         }
     }
-    if (tid == 0) bulk_wait_all();
 }
 
 template <typename T, int N, int SMODE>
