@@ -61,6 +61,7 @@ DESCR = {
     "5": "cfg5 3D Dirac 4 components 256^3, soft-core Coulomb, complex128",
 }
 # 60 % of the 8 TB/s roofline, us per split step; None where the bar does not apply
+OPTIONS = []  # (SSO_OPT_*, value) pairs from --opt, applied to every plan (tuning sweeps)
 BAR_US = {"1": None, "2a": 55.9, "2b": 28.0, "3": 447.4, "4": 28.0, "5": 1789.6}
 
 
@@ -245,6 +246,8 @@ def measure(name, K, W, world, barrier, sampler, want_e2e):
 
     plan = sso.Plan(w.sizes, w.dx, w.dt, w.ncomp, precision)
     plan.set_constants(w.mass, w.c, w.charge)
+    for opt, val in OPTIONS:
+        plan.set_option(opt, val)
     plan.set_potential(w.V)
     if w.field_kind:
         plan.set_field(w.field_kind, np.ascontiguousarray(w.step_avg))
@@ -397,7 +400,11 @@ def main():
     ap.add_argument("--workload", default=HEADLINE, choices=sorted(WORKLOADS), help="headline workload (top-level numbers)")
     ap.add_argument("--only", action="store_true", help="time the headline workload only (no per_workload sweep)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", default="", help="tuning: comma-separated SSO_OPT_<number>=<value> pairs applied to every plan, e.g. 4=2,5=6")
     args = ap.parse_args()
+    for kv in filter(None, args.opt.split(",")):
+        k, v = kv.split("=")
+        OPTIONS.append((int(k), int(v)))
     if args.impl == "reference":
         return run_reference(args)
     return run_product(args)

@@ -74,8 +74,10 @@ extern "C" {
                                             sso_set_potential has been called again                */
 
 #define SSO_OPT_GROUPS_PER_CTA 4         /* independent line groups per CTA (0 = auto)              */
-#define SSO_OPT_RING_BUFFERS 5           /* ring buffers PER GROUP of the ring pipelines (0 = auto: 2 if they fit) */
+#define SSO_OPT_RING_BUFFERS 5           /* tile buffers per CTA of the pass pipelines (0 = auto: as many as fit)  */
 #define SSO_OPT_STRIDED_RING 7           /* strided-axis passes: 0 auto, 1 force the TMA ring, 2 direct kernel only */
+#define SSO_OPT_DIRAC_TABLE 8            /* Dirac plans without a field, ndim >= 2: 0 = cos(E tau), sin(E tau)/E of every k point
+                                            evaluated in the kinetic pass, 1 = read from a table (16 bytes per k point) */
 #define SSO_OPT_THREADS_PER_CTA 6        /* ring pipeline CTA size: 512 (128 regs/thread) or 384 (168); 0 = auto */
 
 #define SSO_MIN_AXIS 16   /* smallest supported axis length                       */

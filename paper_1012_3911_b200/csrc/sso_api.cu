@@ -23,6 +23,7 @@
 
 #include "../../include/sso.h"
 #include "sso_dispatch.h"
+#include "sso_line1d_args.h"
 
 namespace sso {
 
@@ -76,6 +77,29 @@ __global__ void build_kphase_kernel(const double *__restrict__ kv, void *__restr
     h.x = (T)(c * scale);
     h.y = (T)(s * scale);
     reinterpret_cast<C *>(out)[i] = h;
+}
+
+// Dirac kinetic pass tables.  cp0[s] = c (k_0[s] - sh0) for every slot s of axis 0; and, when `out` is given, the
+// kinetic scalars of every k point in the order the pass meets them ([slot along axis 0][the other axes in storage
+// order]):  out = scale * (cos(E tau), sin(E tau)/E),  E = sqrt(c^2 |k - sh|^2 + m^2 c^4), sh = q Abar_n
+// (eq. 32; closed form of eq. 33, see sso_sring.cuh; reading G16 for the shift)
+__global__ void build_ktab_kernel(double2 *__restrict__ out, double *__restrict__ cp0, const double *__restrict__ kv0,
+                                  const double *__restrict__ kv1, const double *__restrict__ kv2, int n0, long long total, long long inner,
+                                  int rest1, double sh0, double sh1, double sh2, double mass, double clight, double dt, double scale) {
+    const long long tid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (tid < n0) cp0[tid] = clight * (kv0[tid] - sh0);
+    if (!out) return;
+    const double mc2 = mass * clight * clight;
+    for (long long i = tid; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const long long s = i / inner, line = i % inner;
+        const double p0 = kv0[s] - sh0;
+        const double p1 = kv1 ? kv1[line / rest1] - sh1 : (kv2 ? kv2[line % rest1] - sh1 : 0.0);
+        const double p2 = kv1 ? kv2[line % rest1] - sh2 : 0.0;
+        const double E = sqrt(clight * clight * (p0 * p0 + p1 * p1 + p2 * p2) + mc2 * mc2);
+        double sn, cs;
+        sincos(E * dt, &sn, &cs);
+        out[i] = make_double2(cs * scale, (E > 0.0 ? sn / E : dt) * scale);
+    }
 }
 
 // homogeneous E field, all passes of one sso_step call at once (2D/3D).  For every lattice axis with a field
@@ -172,6 +196,17 @@ static SRingLaunchFn find_sring(int precision, int N, int mode) {
     return nullptr;
 }
 
+static Line1dLaunchFn find_line1d(int precision, int N) {
+    switch (N) {
+#define SSO_CASE(NN) \
+    case NN:         \
+        return precision == SSO_C64 ? sso_line1d_lookup_f32_##NN() : sso_line1d_lookup_f64_##NN();
+        SSO_FOR_EACH_N(SSO_CASE)
+#undef SSO_CASE
+    }
+    return nullptr;
+}
+
 static RingLaunchFn find_ring(int precision, int N, int mode, int maxt) {
     switch (N) {
 #define SSO_CASE(NN) \
@@ -262,6 +297,10 @@ struct sso_plan {
     int tmap_tl[3] = {0, 0, 0};
     int vrep = VREP_TABLE;
     bool kph_valid = false;
+    void *d_ktab = nullptr;   // Dirac kinetic scalars per k point (SSO_OPT_DIRAC_TABLE = 1), else NULL
+    double *d_kcp0 = nullptr; // Dirac: c (k_0 - q Abar_0) per slot of axis 0
+    bool ktab_valid = false;  // both tables are current (plans without SSO_FIELD_A only; with it they change every step)
+    int opt_dirac_table = 0;
     int opt_tl_contig = 0, opt_tl_strided = 0, opt_groups = 0, opt_ring = 0, opt_maxt = 0, opt_sring = 0;
     int device = 0, num_sms = 0;  // the device the plan was created on, its SM count
     size_t smem_optin = 0;        // largest dynamic shared memory a CTA may opt in to on that device
@@ -503,6 +542,8 @@ int sso_destroy(sso_plan *plan) {
     cudaFree(plan->d_avg);
     cudaFree(plan->d_vtab);
     cudaFree(plan->d_vfull);
+    cudaFree(plan->d_ktab);
+    cudaFree(plan->d_kcp0);
     for (int a = 0; a < 3; ++a) cudaFree(plan->d_erow[a]);
     cudaFree(plan->d_partial);
     cudaFree(plan->d_norm);
@@ -520,6 +561,7 @@ int sso_set_constants(sso_plan *plan, double mass, double c, double charge) {
     plan->clight = c;
     plan->charge = charge;
     plan->kph_valid = false;
+    plan->ktab_valid = false;
     return SSO_OK;
 }
 
@@ -580,6 +622,7 @@ int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nval
         plan->e_along_last = false;
         for (int a = 0; a < 3; ++a) plan->e_axis_on[a] = false;
         plan->kph_valid = false;
+    plan->ktab_valid = false;
         return SSO_OK;
     }
     if (!step_avg || nvals <= 0) return fail(plan, SSO_ERR_INVALID, "step_avg is NULL or nvals <= 0");
@@ -625,6 +668,7 @@ int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nval
         }
     }
     plan->kph_valid = false;
+    plan->ktab_valid = false;
     return SSO_OK;
 }
 
@@ -658,12 +702,21 @@ int sso_set_option(sso_plan *plan, int option, int64_t value) {
             plan->opt_maxt = (int)value;
             return SSO_OK;
         case SSO_OPT_STRIDED_RING:
-            if (value < 0 || value > 4) return fail(plan, SSO_ERR_INVALID, "strided ring mode must be 0 (auto), 1 (force) or 2 (off)");
+            if (value < 0 || value > 2) return fail(plan, SSO_ERR_INVALID, "strided ring mode must be 0 (auto), 1 (force) or 2 (off)");
             plan->opt_sring = (int)value;
             return SSO_OK;
         case SSO_OPT_GROUPS_PER_CTA:
             if (value < 0 || value > 15) return fail(plan, SSO_ERR_INVALID, "groups per CTA must be in [0, 15]");
             plan->opt_groups = (int)value;
+            return SSO_OK;
+        case SSO_OPT_DIRAC_TABLE:
+            if (value != 0 && value != 1) return fail(plan, SSO_ERR_INVALID, "Dirac table mode must be 0 or 1");
+            plan->opt_dirac_table = (int)value;
+            if (!value) {
+                cudaFree(plan->d_ktab);
+                plan->d_ktab = nullptr;
+            }
+            plan->ktab_valid = false;
             return SSO_OK;
         case SSO_OPT_POTENTIAL_PHASE:
             if (value != VREP_TABLE && value != VREP_ANGLE) return fail(plan, SSO_ERR_INVALID, "potential phase mode must be 0 or 1");
@@ -947,47 +1000,70 @@ struct SRingShape {
     size_t bufbytes, twbytes;
 };
 
-// tile shape of a strided pass, or ok = false when the ring does not fit (the direct kernel takes over)
-SRingShape sring_shape(const sso_plan *plan, int axis, int cc) {
+// tile shape of a strided pass, or ok = false when the pool does not fit (the direct kernel takes over).
+// `light` marks the transform-only passes of the middle axis, which need fewer compute groups per byte moved.
+SRingShape sring_shape(const sso_plan *plan, int axis, int cc, bool light) {
+    const int smode = light ? SMODE_DIF : (cc == 1 ? SMODE_KS : SMODE_KD4);
     SRingShape r{};
     if (plan->opt_sring == 2 || !encode_tiled_fn()) return r;
     const Axis &A = plan->ax[axis];
     const Geometry g = geometry(plan, axis);
     const int U = A.n / 16, esz = (int)plan->esize();
-    // rows of 128 bytes when two or more buffers of such tiles fit; else narrower rows (TMA serves 32-byte rows
-    // better than per-thread loads do), down to one buffer holding the widest tile that fits
-    const int Gn = 128 / esz;
+    const int Gn = 128 / esz;  // complex numbers per 128 bytes
+    // twiddles + the pass's line table come first in shared memory; 256 bytes hold the pool's barriers and mailboxes
+    const size_t tw = (size_t)twiddle_count_padded(A.n) * esz + (size_t)sring_line_table_bytes(smode, A.n, esz);
+    if (tw + 256 >= plan->smem_optin) return r;
+    const size_t room = plan->smem_optin - 256 - tw;
+    auto pitch_of = [&](int TL) { return A.n + A.n / 16 + (Gn / TL > 1 ? Gn / TL : 1); };
+    auto bufbytes_of = [&](int TL) { return ((size_t)cc * TL * pitch_of(TL) * esz + 127) & ~(size_t)127; };
+    // a tile shape is usable when whole warps make a group, a row is at least 16 bytes, and the cc components of a
+    // k point fall into one warp (thread layout of sso_sring.cuh)
     auto fits = [&](int TL, int *bmax_out) {
-        if (TL < 1 || TL > g.inner || g.inner % TL != 0 || cc * TL * U > 512 || (cc * TL * U) % 32 != 0) return false;
-        const int pitch = A.n + A.n / 16 + (Gn / TL > 1 ? Gn / TL : 1);
-        const size_t bb = ((size_t)cc * TL * pitch * esz + 127) & ~(size_t)127;
-        const size_t tw = (size_t)twiddle_count_padded(A.n) * esz;
-        if (bb + tw > (size_t)plan->smem_optin - 256) return false;
-        *bmax_out = (int)(((size_t)plan->smem_optin - 256 - tw) / bb);
+        if (TL < 1 || TL > g.inner || g.inner % TL != 0 || TL * esz < 16) return false;
+        const int GT = cc * TL * U;
+        if (GT > 512 || GT % 32 != 0) return false;
+        const int UL = TL >= 8 ? 1 : (8 / TL < U ? 8 / TL : U);
+        if (cc * TL * UL > 32 || U % UL != 0) return false;
+        const size_t bb = bufbytes_of(TL);
+        if (bb > room) return false;
+        *bmax_out = (int)(room / bb);
         return true;
     };
     int TL = 0, bm = 0;
     if (plan->opt_tl_strided > 0) {
         if (fits(plan->opt_tl_strided, &bm)) TL = plan->opt_tl_strided;
     } else {
-        for (int cand = 128 / esz; cand >= 32 / esz && cand >= 1 && !TL; cand /= 2)
-            if (fits(cand, &bm) && bm >= 2) TL = cand;
-        for (int cand = 128 / esz; cand >= 32 / esz && cand >= 1 && !TL; cand /= 2)
-            if (fits(cand, &bm)) TL = cand;
+        // the widest rows (up to 128 bytes) that leave room for two buffers or more
+        for (int want = 2; want >= 1 && !TL; --want)
+            for (int cand = Gn; cand >= 1 && !TL; cand /= 2)
+                if (fits(cand, &bm) && bm >= want) TL = cand;
     }
     if (!TL) return r;
     r.TL = TL;
     r.GT = cc * TL * U;
-    r.pitch = A.n + A.n / 16 + (Gn / TL > 1 ? Gn / TL : 1);
-    r.bufbytes = ((size_t)cc * TL * r.pitch * esz + 127) & ~(size_t)127;
-    r.twbytes = (size_t)twiddle_count_padded(A.n) * esz;
-    const int bmax = (int)(((size_t)plan->smem_optin - 256 - r.twbytes) / r.bufbytes);
-    if (bmax < 1) return r;
-    int NBG = 1;
+    r.pitch = pitch_of(TL);
+    r.bufbytes = bufbytes_of(TL);
+    r.twbytes = tw;
+    int bmax = (int)(room / r.bufbytes);
+    if (bmax > 12) bmax = 12;
     const long long outer = plan->npts / (A.n * g.inner);
     const long long ntiles = (cc == 1 ? outer * plan->ncomp : 1) * (g.inner / TL);
-    choose_groups(plan, r.GT, bmax, (ntiles + plan->num_sms - 1) / plan->num_sms, &r.G, &NBG);
-    r.NB = r.G * NBG;
+    const long long per_cta = (ntiles + plan->num_sms - 1) / plan->num_sms;
+    // as many groups as threads and buffers allow; the buffers left over go round the groups (a group with two
+    // buffers loads its next tile while it works).  The transform-only passes run at HBM speed single-buffered and
+    // measured slightly slower with more loads in flight, so they get one buffer per group.
+    int G = 512 / r.GT;
+    if (plan->opt_groups > 0 && plan->opt_groups < G) G = plan->opt_groups;
+    if (G > bmax) G = bmax;
+    if (G > per_cta) G = (int)per_cta;
+    if (G > 15) G = 15;
+    if (G < 1) G = 1;
+    int NB = light ? G : bmax;
+    if (NB > 2 * G) NB = 2 * G;
+    if (plan->opt_ring > 0 && plan->opt_ring < NB) NB = plan->opt_ring;
+    if (NB < G) NB = G;
+    r.G = G;
+    r.NB = NB;
     r.box_rows = A.n < 256 ? A.n : 256;
     r.ok = true;
     return r;
@@ -1046,10 +1122,13 @@ int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long 
         a.kv2 = g.oaxB >= 0 ? plan->ax[g.oaxB].d_kv : nullptr;
         if (plan->field_kind == SSO_FIELD_A)
             for (int ax = 0; ax < plan->ndim; ++ax) a.sh[ax] = plan->charge * plan->h_avg[(size_t)n * plan->ndim + ax];
+        a.kcp0 = plan->d_kcp0;
+        a.ktab = plan->d_ktab;
+        if (!plan->opt_dirac_table) smode = smode == SMODE_KD2 ? SMODE_KD2F : SMODE_KD4F;
     }
     SRingLaunchFn fn = find_sring(plan->precision, A.n, smode);
     if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no strided ring kernel built for this line length");
-    const size_t smem = sh.twbytes + (size_t)sh.NB * sh.bufbytes + (size_t)sh.NB * 8 + (size_t)(sh.NB + 1) * 4;
+    const size_t smem = sh.twbytes + (size_t)sh.NB * sh.bufbytes + (size_t)sh.NB * 12 + 4;
     const unsigned grid = (unsigned)(ntiles < plan->num_sms ? ntiles : plan->num_sms);
     cudaError_t e = fn(a, &plan->tmap[axis], (unsigned)(a.G * sh.GT), smem, grid, st);
     return pass_status(plan, smode == SMODE_DIF ? "strided ring DIF pass" : (smode == SMODE_DIT ? "strided ring DIT pass" : "strided ring kinetic pass"), e);
@@ -1115,6 +1194,37 @@ int build_kphase(sso_plan *plan, long long n, cudaStream_t st) {
     return SSO_OK;
 }
 
+// tables of the Dirac kinetic pass (build_ktab_kernel): built once for a plan without SSO_FIELD_A, every step with it
+bool dirac_tables_per_step(const sso_plan *p) { return p->ncomp > 1 && p->ndim >= 2 && p->field_kind == SSO_FIELD_A; }
+int build_ktab(sso_plan *plan, long long n, cudaStream_t st) {
+    if (plan->ncomp == 1 || plan->ndim < 2) return SSO_OK;
+    const bool shifted = plan->field_kind == SSO_FIELD_A;
+    if (plan->ktab_valid && !shifted) return SSO_OK;
+    if (!plan->d_kcp0) {
+        cudaError_t e = cudaMalloc((void **)&plan->d_kcp0, sizeof(double) * (size_t)plan->ax[0].n);
+        if (e != cudaSuccess) return fail(plan, SSO_ERR_ALLOC, std::string("Dirac momentum table: ") + cudaGetErrorString(e));
+    }
+    if (plan->opt_dirac_table && !plan->d_ktab) {
+        cudaError_t e = cudaMalloc(&plan->d_ktab, sizeof(double2) * (size_t)plan->npts);
+        if (e != cudaSuccess) return fail(plan, SSO_ERR_ALLOC, std::string("Dirac kinetic table: ") + cudaGetErrorString(e));
+    }
+    double sh[3] = {0.0, 0.0, 0.0};
+    if (shifted)
+        for (int ax = 0; ax < plan->ndim; ++ax) sh[ax] = plan->charge * plan->h_avg[(size_t)n * plan->ndim + ax];
+    PassTimer timer(plan, SSO_PASS_TABLES, st);
+    const Geometry g = geometry(plan, 0);
+    const bool table = plan->opt_dirac_table != 0;
+    const int blocks = table ? plan->num_sms * 8 : (plan->ax[0].n + 255) / 256;
+    build_ktab_kernel<<<blocks, 256, 0, st>>>(table ? reinterpret_cast<double2 *>(plan->d_ktab) : nullptr, plan->d_kcp0, plan->ax[0].d_kv,
+                                             g.oaxA >= 0 ? plan->ax[g.oaxA].d_kv : nullptr, g.oaxB >= 0 ? plan->ax[g.oaxB].d_kv : nullptr,
+                                             plan->ax[0].n, plan->npts, g.inner, g.rest1, sh[0], sh[1], sh[2], plan->mass, plan->clight, plan->dt,
+                                             1.0 / (double)plan->npts);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(plan, e, "Dirac kinetic table kernel");
+    plan->ktab_valid = !shifted;
+    return SSO_OK;
+}
+
 int kinetic_pw(const sso_plan *p) { return p->ncomp == 1 ? PW_KS : (p->ncomp == 2 ? PW_KD2 : PW_KD4); }
 
 long long launches_for(const sso_plan *p, long long nsteps) {
@@ -1128,6 +1238,7 @@ long long launches_for(const sso_plan *p, long long nsteps) {
     }
     const long long chunk = erow_chunk(p);
     const long long nchunks = (nsteps + chunk - 1) / chunk;
+    if (p->ncomp > 1 && sring_shape(p, 0, p->ncomp, false).ok) cnt += dirac_tables_per_step(p) ? nsteps : (p->ktab_valid ? 0 : 1);  // Dirac kinetic tables
     bool eph = false;
     for (int a = 0; a < p->ndim; ++a) eph = eph || (p->field_kind == SSO_FIELD_E && p->e_axis_on[a]);
     cnt += nchunks * (eph ? 2 : 1);              // opening pass (+ field phase rows)
@@ -1169,17 +1280,32 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
         const long long chunk = kshift ? 1 : nsteps;  // step-dependent kinetic tables force one launch per step
         for (long long s = 0; s < nsteps; s += chunk) {
             if (plan->ncomp == 1 && (rc = build_kphase(plan, n0 + s, st)) != SSO_OK) return rc;
-            PassSpec ps{0, kpw, -1, 1, 1, 0, 1, 1, 1, (int)chunk, n0 + s};
             if (chunk > 0x7fffffffLL) return fail(plan, SSO_ERR_INVALID, "nsteps too large");
+            Line1dLaunchFn l1 = (plan->ncomp == 1 && plan->field_kind != SSO_FIELD_E) ? find_line1d(plan->precision, plan->ax[0].n) : nullptr;
+            if (l1) {
+                // Schroedinger without a length-gauge field: both pointwise tables are constant over the launch and
+                // live in registers (sso_line1d.cuh)
+                PassTimer timer(plan, SSO_PASS_LINE_1D, st);
+                Line1dArgs la{};
+                la.psi = psi;
+                la.tw = plan->ax[0].tw;
+                la.vtab = plan->d_vtab;
+                la.vrep = plan->vrep;
+                la.kph0 = plan->ax[0].d_kph;
+                la.nsteps = (int)chunk;
+                const int n = plan->ax[0].n;
+                const size_t smem = ((size_t)twiddle_count_padded(n) + n + n / 16) * plan->esize();
+                if ((rc = pass_status(plan, "1D line kernel", l1(la, smem, st))) != SSO_OK) return rc;
+                continue;
+            }
+            PassSpec ps{0, kpw, -1, 1, 1, 0, 1, 1, 1, (int)chunk, n0 + s};
             if ((rc = launch(plan, psi, ps, st)) != SSO_OK) return rc;
         }
     } else {
         // chunks that share one set of field phase rows; each chunk opens and closes with a half step
         const long long chunk = erow_chunk(plan);
-        SRingShape shk = sring_shape(plan, 0, plan->ncomp == 1 ? 1 : plan->ncomp);
-        SRingShape shm = nd == 3 ? sring_shape(plan, 1, 1) : SRingShape{};
-        if (plan->opt_sring == 3) shm.ok = false;  // development: kinetic pass only
-        if (plan->opt_sring == 4) shk.ok = false;  // development: middle-axis passes only
+        SRingShape shk = sring_shape(plan, 0, plan->ncomp == 1 ? 1 : plan->ncomp, false);
+        SRingShape shm = nd == 3 ? sring_shape(plan, 1, 1, true) : SRingShape{};
         for (long long c0 = 0; c0 < nsteps; c0 += chunk) {
             const long long ns = nsteps - c0 < chunk ? nsteps - c0 : chunk;
             const long long nb = n0 + c0;
@@ -1197,6 +1323,7 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
                     }
                     if (rc != SSO_OK) return rc;
                 }
+                if (shk.ok && (rc = build_ktab(plan, n, st)) != SSO_OK) return rc;
                 if (shk.ok) rc = launch_sring_pass(plan, psi, 0, kpw == PW_KS ? SMODE_KS : (kpw == PW_KD2 ? SMODE_KD2 : SMODE_KD4), n, shk, st);
                 else {
                     PassSpec kin{0, kpw, -1, 1, 1, 0, 1, 0, 0, 1, n};  // F_0 K F_0^-1

@@ -93,7 +93,8 @@ struct RingArgs {
 using RingLaunchFn = cudaError_t (*)(const RingArgs &, unsigned threads, size_t smem, unsigned grid, cudaStream_t st);
 
 // strided-axis passes through the same ring, tiles moved as TMA tensor boxes (sso_sring.cuh)
-enum : int { SMODE_KS = 0, SMODE_KD2 = 1, SMODE_KD4 = 2, SMODE_DIF = 3, SMODE_DIT = 4 };
+// KD2 / KD4 read the Dirac kinetic scalars from a table, KD2F / KD4F evaluate them in the pass ("on the fly")
+enum : int { SMODE_KS = 0, SMODE_KD2 = 1, SMODE_KD4 = 2, SMODE_DIF = 3, SMODE_DIT = 4, SMODE_KD2F = 5, SMODE_KD4F = 6 };
 struct SRingArgs {
     void *psi;                // device base of psi (stores from registers; loads go through the tensor map)
     long long inner;          // element stride along the line
@@ -102,7 +103,7 @@ struct SRingArgs {
     int ntiles;               // tiles of TL adjacent lines (x all components when they are independent)
     int TL;                   // adjacent lines per tile: one row of a tile is TL complex numbers, contiguous in memory
     int pitch;                // padded line pitch of the exchange layout (complex elements)
-    int G, GT, NB, bufstride; // as in RingArgs; GT = CC * TL * N/16
+    int G, GT, NB, bufstride; // groups, threads per group (CC * TL * N/16), pool buffers (any number >= 1), elements between buffers
     int tiles_per_outer;      // inner / TL
     int box_rows;             // rows per TMA box (<= 256); a tile is CC * N / box_rows boxes
     int rest1;                // line = ia * rest1 + ib on the non-line axes
@@ -110,9 +111,16 @@ struct SRingArgs {
     const void *kph0, *kph1, *kph2;  // Schroedinger phase tables (PassArgs)
     const double *kv0, *kv1, *kv2;   // Dirac k grids (PassArgs)
     double sh[3];                    // q Abar_n per axis (SSO_FIELD_A), else 0
+    const void *ktab;                // Dirac table modes: double2 (cos(E tau), sin(E tau)/E) / Ntot per k point, [slot of axis 0][inner]
+    const double *kcp0;              // Dirac: c (k_0 - q Abar_0) per slot of axis 0
     double mass, clight, dt, scale;
     int ndim;
 };
+// bytes of the line table a strided pass keeps in shared memory (multiple of 128): the Schroedinger kinetic phases
+// of the line axis (complex[N]) or the Dirac momenta c (k_0 - q Abar_0) (double[N])
+__host__ __device__ constexpr int sring_line_table_bytes(int smode, int N, int esz) {
+    return smode == SMODE_KS ? (N * esz + 127) / 128 * 128 : ((smode == SMODE_DIF || smode == SMODE_DIT) ? 0 : (N * 8 + 127) / 128 * 128);
+}
 using SRingLaunchFn = cudaError_t (*)(const SRingArgs &, const void *tensor_map, unsigned threads, size_t smem, unsigned grid, cudaStream_t st);
 #define SSO_DECL_SRING(N)                            \
     SRingLaunchFn sso_sring_lookup_f32_##N(int mode); \
@@ -124,5 +132,14 @@ SSO_FOR_EACH_N(SSO_DECL_SRING)
     RingLaunchFn sso_ring_lookup_f64_##N(int mode, int maxt);
 SSO_FOR_EACH_N(SSO_DECL_RING)
 #undef SSO_DECL_RING
+
+// the persistent 1D Schroedinger kernel of sso_line1d.cuh
+struct Line1dArgs;
+using Line1dLaunchFn = cudaError_t (*)(const Line1dArgs &, size_t smem, cudaStream_t st);
+#define SSO_DECL_LINE1D(N)                      \
+    Line1dLaunchFn sso_line1d_lookup_f32_##N(); \
+    Line1dLaunchFn sso_line1d_lookup_f64_##N();
+SSO_FOR_EACH_N(SSO_DECL_LINE1D)
+#undef SSO_DECL_LINE1D
 
 }  // namespace sso

@@ -7,6 +7,7 @@
 #include "sso_pass.cuh"
 #include "sso_ring.cuh"
 #include "sso_sring.cuh"
+#include "sso_line1d.cuh"
 #include "sso_dispatch.h"
 
 #ifndef SSO_T
@@ -91,6 +92,15 @@ cudaError_t launch_sring(const SRingArgs &a, const void *tensor_map, unsigned th
     return launch_pdl(kern, grid, threads, smem, st, a, *reinterpret_cast<const CUtensorMap *>(tensor_map));
 }
 
+template <typename T, int N> cudaError_t launch_line1d(const Line1dArgs &a, size_t smem, cudaStream_t st) {
+    auto kern = line1d_kernel<T, N>;
+    static std::atomic<unsigned long long> done{0};
+    cudaError_t e = opt_in_smem(kern, done);
+    if (e != cudaSuccess) return e;
+    kern<<<1, N / 16, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
 #define SSO_CAT3_(a, b, c) a##b##_##c
 #define SSO_CAT3(a, b, c) SSO_CAT3_(a, b, c)
 
@@ -105,10 +115,18 @@ SRingLaunchFn SSO_CAT4(sso_sring_lookup_, SSO_TNAME, SSO_N)(int mode) {
     if (mode == SMODE_KS) return &launch_sring<T, N, SMODE_KS>;
     if (mode == SMODE_KD2) return &launch_sring<T, N, SMODE_KD2>;
     if (mode == SMODE_KD4) return &launch_sring<T, N, SMODE_KD4>;
+    if (mode == SMODE_KD2F) return &launch_sring<T, N, SMODE_KD2F>;
+    if (mode == SMODE_KD4F) return &launch_sring<T, N, SMODE_KD4F>;
     if (mode == SMODE_DIF) return &launch_sring<T, N, SMODE_DIF>;
     if (mode == SMODE_DIT) return &launch_sring<T, N, SMODE_DIT>;
     return nullptr;
 }
+#endif
+
+#ifdef SSO_STUB
+Line1dLaunchFn SSO_CAT4(sso_line1d_lookup_, SSO_TNAME, SSO_N)() { return nullptr; }
+#else
+Line1dLaunchFn SSO_CAT4(sso_line1d_lookup_, SSO_TNAME, SSO_N)() { return &launch_line1d<SSO_T, SSO_N>; }
 #endif
 
 #ifdef SSO_STUB

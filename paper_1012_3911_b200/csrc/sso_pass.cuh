@@ -244,7 +244,12 @@ constexpr int GB_LANES_ARE_U = 1 << 30;
 constexpr int GB_TL_SHIFT = 26;
 
 // registers (layout of stage IA) -> shared memory -> registers (layout of stage IB)
-template <typename T, int N, int IA, int IB> __device__ __forceinline__ void exchange(typename CxOf<T>::type (&x)[16], int u, typename CxOf<T>::type *sl, int gb) {
+struct NoGapWork {
+    __device__ __forceinline__ void operator()() const {}
+};
+// `gap` runs between the writes and the reads, i.e. while the registers of x are free
+template <typename T, int N, int IA, int IB, typename GAP = NoGapWork>
+__device__ __forceinline__ void exchange(typename CxOf<T>::type (&x)[16], int u, typename CxOf<T>::type *sl, int gb, GAP gap = GAP()) {
     using C = typename CxOf<T>::type;
     constexpr int MiA = Sched<N>::nprev(IA) / 16, MiB = Sched<N>::nprev(IB) / 16;
     constexpr int SCOPE = MiA > MiB ? MiA : MiB;
@@ -257,17 +262,22 @@ template <typename T, int N, int IA, int IB> __device__ __forceinline__ void exc
     for (int q = 0; q < 16; ++q) wa[stage_delta<N, IA>(q)] = x[q];
     if (warp_local) __syncwarp();
     else gsync(gb);
+    gap();
 #pragma unroll
     for (int q = 0; q < 16; ++q) x[q] = rb[stage_delta<N, IB>(q)];
 }
 
+// `gap` is work that does not touch x (e.g. the scalars of the pointwise factor): it runs inside the last exchange,
+// when x sits in shared memory and its registers are free (before the only stage when the line has one stage)
 template <typename T, int N, int I, int SIGN> struct DifChain {
     using C = typename CxOf<T>::type;
-    static __device__ __forceinline__ void run(C (&x)[16], int u, const C *tw, C *sl, int gb) {
+    template <typename GAP = NoGapWork> static __device__ __forceinline__ void run(C (&x)[16], int u, const C *tw, C *sl, int gb, GAP gap = GAP()) {
+        if constexpr (Sched<N>::M == 1) gap();
         dif_stage<T, N, I, SIGN>(x, u, tw);
         if constexpr (I + 1 < Sched<N>::M) {
-            exchange<T, N, I, I + 1>(x, u, sl, gb);
-            DifChain<T, N, I + 1, SIGN>::run(x, u, tw, sl, gb);
+            if constexpr (I + 2 == Sched<N>::M) exchange<T, N, I, I + 1>(x, u, sl, gb, gap);
+            else exchange<T, N, I, I + 1>(x, u, sl, gb);
+            DifChain<T, N, I + 1, SIGN>::run(x, u, tw, sl, gb, gap);
         }
     }
 };
@@ -286,6 +296,41 @@ template <typename T, int N, int I, int SIGN> struct DitChain {  // runs stages 
 template <typename T> __device__ __forceinline__ typename CxOf<T>::type expi(double a) {
     double s, c;
     sincos(a, &s, &c);
+    return mk<typename CxOf<T>::type>((T)c, (T)s);
+}
+
+// exp(i a) for |a| <= 4 pi, evaluated in double without the library's general argument reduction: the plan stores
+// potential angles reduced to [-pi, pi] (VREP_ANGLE), so a quadrant reduction j = rint(2a/pi), r = a - j pi/2 with a
+// two-term pi/2 and the Taylor polynomials of sin and cos on [-pi/4, pi/4] (truncation error r^17/17! < 5e-17,
+// r^18/18! < 3e-18) are enough.  About 24 FP64 instructions against about 45 for sincos().
+template <typename T> __device__ __forceinline__ typename CxOf<T>::type expi_small(double a) {
+    const double magic = 6755399441055744.0;  // 1.5 * 2^52: adding it rounds to the nearest integer, kept in the low bits
+    const double jm = fma(a, 0.63661977236758134308, magic);
+    const int j = __double2loint(jm);
+    const double jd = jm - magic;
+    double r = fma(jd, -1.57079632679489655800e+00, a);   // pi/2, leading 53 bits
+    r = fma(jd, -6.12323399573676603587e-17, r);          // pi/2, next bits
+    const double z = r * r;
+    double sp = fma(z, -1.0 / 1307674368000.0, 1.0 / 6227020800.0);
+    sp = fma(z, sp, -1.0 / 39916800.0);
+    sp = fma(z, sp, 1.0 / 362880.0);
+    sp = fma(z, sp, -1.0 / 5040.0);
+    sp = fma(z, sp, 1.0 / 120.0);
+    sp = fma(z, sp, -1.0 / 6.0);
+    const double sn = fma(r * z, sp, r);
+    double cp = fma(z, 1.0 / 20922789888000.0, -1.0 / 87178291200.0);
+    cp = fma(z, cp, 1.0 / 479001600.0);
+    cp = fma(z, cp, -1.0 / 3628800.0);
+    cp = fma(z, cp, 1.0 / 40320.0);
+    cp = fma(z, cp, -1.0 / 720.0);
+    cp = fma(z, cp, 1.0 / 24.0);
+    cp = fma(z, cp, -0.5);
+    const double cs = fma(z, cp, 1.0);
+    // quadrant j mod 4: (cos, sin) -> (cs, sn), (-sn, cs), (-cs, -sn), (sn, -cs)
+    double c = (j & 1) ? sn : cs;
+    double s = (j & 1) ? cs : sn;
+    if ((j + 1) & 2) c = -c;
+    if (j & 2) s = -s;
     return mk<typename CxOf<T>::type>((T)c, (T)s);
 }
 
@@ -507,7 +552,7 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
                         if (full) h = cmul(h, h);
                     } else {
                         const double ang = reinterpret_cast<const double *>(a.vtab)[vi];
-                        h = expi<T>(full ? 2.0 * ang : ang);
+                        h = expi_small<T>(full ? 2.0 * ang : ang);
                     }
                     if (a.field_kind == 1) {
                         const double r = ((double)(u + q * U) - (double)(N / 2)) * a.dxs[a.line_axis];
@@ -564,7 +609,6 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
                         x[q] = cmul(x[q], f);
                     }
                 } else if constexpr (PW == PW_KD2 || PW == PW_KD4) {
-                    constexpr int PP = 16 / CC;
                     // shift of the kinetic momentum: pi = k - q Abar_n (reading G16)
                     double sh[3] = {0.0, 0.0, 0.0};
                     if (a.field_kind == 2)

@@ -78,12 +78,61 @@ __device__ __forceinline__ double ld_table(const double *p, uint64_t pol) {
     asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
     return v;
 }
+// plain streamed table load (read once per pass, shared by the lanes of a k point)
+__device__ __forceinline__ double2 ld_table(const double2 *p) {
+    double2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ void prefetch_l2_bulk_hint(const void *p, unsigned bytes, uint64_t pol) {
     asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(p), "r"(bytes), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void prefetch_l2_bulk_plain(const void *p, unsigned bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
+
+// Tile buffers of a persistent CTA: NB shared-memory buffers, G compute groups, buffer b owned by group b mod G
+// (so a group owns NB / G buffers, the first NB mod G groups one more).  A group's leader fills its buffers, its
+// threads consume them in turn, so a buffer's mbarrier never sees a waiter that is not in step with its fills
+// (a ring shared between groups let a fast group wait on a buffer one fill ahead of its phase, and an in-order
+// shared queue made fast groups wait for slow ones).  Which tile a buffer gets next is decided when the buffer is
+// refilled, from a counter shared by the CTA: the tiles are spread evenly whatever their count, and a group with
+// more buffers simply works through more tiles.
+struct TileRing {
+    unsigned long long *bar;  // [NB] "tile landed" barriers
+    volatile int *kt;         // [NB] tile held by each buffer, -1: none left
+    int *next;                // next unclaimed tile of the CTA
+    int NB, G;
+    __device__ TileRing(void *base, int nb, int g) : NB(nb), G(g) {
+        bar = reinterpret_cast<unsigned long long *>(base);
+        kt = reinterpret_cast<volatile int *>(bar + nb);
+        next = const_cast<int *>(kt + nb);
+    }
+    static __host__ __device__ size_t bytes(int nb) { return (size_t)nb * 12 + 4; }
+    __device__ void *full(int b) const { return bar + b; }
+    // once per CTA, by thread 0, before the __syncthreads that precedes the first fill
+    __device__ void init() const {
+        if (threadIdx.x == 0) {
+            for (int b = 0; b < NB; ++b) mbar_init(bar + b, 1);
+            *next = NB;  // tiles 0 .. NB-1 go to buffers 0 .. NB-1
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+    }
+    __device__ int owned(int grp) const { return (NB - grp + G - 1) / G; }            // buffers of this group
+    __device__ int buffer(int grp, int j) const { return grp + G * (j % owned(grp)); }  // buffer of its j-th tile
+    // blocks until the group's j-th fill has landed; returns the tile (-1: no tiles left)
+    __device__ int wait(int grp, int j) const {
+        const int nb = owned(grp), b = grp + G * (j % nb);
+        mbar_wait(bar + b, (unsigned)((j / nb) & 1));
+        return kt[b];
+    }
+    __device__ int claim() const { return atomicAdd(next, 1); }
+    // a buffer with no tile left completes its phase by hand so that its group sees the end
+    __device__ void mark(int b, int k, int nloc) const {
+        kt[b] = k < nloc ? k : -1;
+        if (k >= nloc) mbar_arrive(bar + b);
+    }
+};
 
 template <typename T, int N, int MODE, int SIGN, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
@@ -228,7 +277,7 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
                 const double *vt = reinterpret_cast<const double *>(a.vtab) + vbase;
 #pragma unroll
                 for (int q = 0; q < 16; ++q) {
-                    C f = expi<T>(ld_table(vt + q * U, pol));
+                    C f = expi_small<T>(ld_table(vt + q * U, pol));
                     if (a.eline) f = cmul(f, reinterpret_cast<const C *>(a.eline)[q * U + u]);
                     if (has_s) f = cmul(f, s);
                     x[q] = cmul(x[q], f);

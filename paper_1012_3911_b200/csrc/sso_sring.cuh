@@ -1,14 +1,18 @@
-// sso_sring.cuh -- strided-axis passes of a 2D/3D lattice through the ring pipeline of sso_ring.cuh (sm_100a).
+// sso_sring.cuh -- strided-axis passes of a 2D/3D lattice through the tile rings of sso_ring.cuh (sm_100a).
 //
 // Along a non-last axis the elements of a line are `inner` apart, so a tile is TL ADJACENT lines: N rows of
-// TL contiguous complex numbers (TL * sizeof(complex) >= 64 bytes per row, B200 serves narrower rows at less
-// than half speed).  The TMA engine moves such a tile as tensor boxes (cp.async.bulk.tensor, SASS
-// UTMALDG/UTMASTG) between global memory and a ring buffer laid out [component][row][TL]; everything else is
-// the ring of sso_ring.cuh.  Passes:
+// TL contiguous complex numbers.  The TMA engine loads such a tile as tensor boxes (cp.async.bulk.tensor, SASS
+// UTMALDG) into a ring buffer laid out [component][row][TL]; the results are stored from registers.  Passes:
 //
 //   SMODE_KS / KD2 / KD4   forward DIF -> kinetic factor -> inverse DIT     (eq. 13; 203-232 eq. 27-33)
 //   SMODE_DIF              forward DIF, result left in network order         (middle axis of a 3D lattice)
 //   SMODE_DIT              inverse DIT from network order
+//
+// Thread layout of a group (GT = CC * TL * N/16 threads, CC = components worked on together): with UL = 8 / TL,
+//   tid = t + TL * (ulo + UL * (c + CC * uhi)),   u = ulo + UL * uhi,
+// so that a quarter warp reads 128 contiguous bytes of the tile and the CC components of a k point sit in lanes
+// of one warp: the Dirac kinetic factor gathers them through the exchange buffer with warp-level
+// synchronisation only (a version that traded them with shuffles, 224 SHFL per thread and tile, measured slower).
 #pragma once
 #include <cuda.h>
 
@@ -23,29 +27,126 @@ __device__ __forceinline__ void tma_load_3d(void *smem_dst, const CUtensorMap *m
                  : "memory");
 }
 
+// Thread (c, u) of a line applies the factor to the PP = 16/CC k points of slots (c PP + i) U + u, all components:
+template <int CC> struct DiracScalars {
+    double cs[16 / CC], sE[16 / CC];  // cos(E tau) / Ntot and sin(E tau) / (E Ntot) of those k points
+};
+// evaluated while x is parked in shared memory (inside the last exchange of the forward transform), so that sqrt and
+// sincos run with the registers of x free.  r12 = c^2 (pi_1^2 + pi_2^2) + m^2 c^4 is the same for the whole line.
+template <int CC, int U>
+__device__ __forceinline__ void dirac_scalars(DiracScalars<CC> &k, int u, int c, const double *cp0, double r12, double dt, double scale) {
+    constexpr int PP = 16 / CC;
+#pragma unroll
+    for (int i = 0; i < PP; ++i) {
+        const double w0 = cp0[(c * PP + i) * U + u];
+        const double E = sqrt(w0 * w0 + r12);
+        double sn, cs;
+        sincos(E * dt, &sn, &cs);
+        k.cs[i] = cs * scale;
+        k.sE[i] = (E > 0.0 ? sn / E : dt) * scale;
+    }
+}
+
+// Dirac kinetic factor on the DIF output (eq. 27-33, 240-242 eq. 35) in the closed form
+//   U = cos(E tau) - i (sin(E tau)/E) (c alpha.pi + m c^2 beta),   E = sqrt(c^2 pi^2 + m^2 c^4),
+// which follows from H^2 = E^2 by the argument of PAPER.md:168-184 (eq. 23/24).  The CC components of a k point
+// are gathered into one thread through the exchange buffer, multiplied by the 2x2 / 4x4 unitary and scattered back.
+// The CC threads that trade values are lanes of one warp (thread layout of the kernel), so the two hand-overs need
+// a __syncwarp each and no group barrier.  `me` = this thread's 16 slots of its own line (stage layout of the last
+// stage), `line0` = the same line of component 0, comp_pitch = elements between components.
+//   TABLE: cs, sE come from the table `ktab` instead of `k`.
+template <typename T, int CC, int U, bool TABLE>
+__device__ __forceinline__ void dirac_kinetic_warp(typename CxOf<T>::type (&x)[16], int u, int c, typename CxOf<T>::type *me, typename CxOf<T>::type *line0,
+                                                   int comp_pitch, const double *cp0, double w1, double w2, double mc2, const DiracScalars<CC> &k,
+                                                   const double2 *__restrict__ ktab, long long ktab_stride) {
+    using C = typename CxOf<T>::type;
+    constexpr int PP = 16 / CC;
+#pragma unroll
+    for (int q = 0; q < 16; ++q) me[q] = x[q];
+    __syncwarp();
+    C y[CC][PP];
+#pragma unroll
+    for (int c2 = 0; c2 < CC; ++c2)
+#pragma unroll
+        for (int i = 0; i < PP; ++i) y[c2][i] = line0[c2 * comp_pitch + 17 * u + c * PP + i];
+#pragma unroll
+    for (int i = 0; i < PP; ++i) {
+        const int slot = (c * PP + i) * U + u;
+        double cs, sE;
+        if constexpr (TABLE) {
+            const double2 e = ld_table(ktab + (long long)slot * ktab_stride);
+            cs = e.x;
+            sE = e.y;
+        } else {
+            cs = k.cs[i];
+            sE = k.sE[i];
+        }
+        const T fc = (T)cs;
+        const T fm = (T)(sE * mc2);
+        const T f0 = (T)(sE * cp0[slot]), f1 = (T)(sE * w1), f2 = (T)(sE * w2);
+        // out = cs psi - i sE H psi ;  (-i)(a + i b) = b - i a
+        if constexpr (CC == 2) {
+            const C a0 = y[0][i], a1 = y[1][i];
+            // H psi_0 = mc2 a0 + c (p0 - i p1) a1 ; H psi_1 = c (p0 + i p1) a0 - mc2 a1
+            const C h0 = mk<C>(fm * a0.x + f0 * a1.x + f1 * a1.y, fm * a0.y + f0 * a1.y - f1 * a1.x);
+            const C h1 = mk<C>(f0 * a0.x - f1 * a0.y - fm * a1.x, f0 * a0.y + f1 * a0.x - fm * a1.y);
+            y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
+            y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
+        } else {
+            const C a0 = y[0][i], a1 = y[1][i], a2 = y[2][i], a3 = y[3][i];
+            // sigma.p (v0, v1) = (p2 v0 + (p0 - i p1) v1, (p0 + i p1) v0 - p2 v1)
+            // H psi = (mc2 u + c sigma.p l, c sigma.p u - mc2 l)
+            const C h0 = mk<C>(fm * a0.x + f2 * a2.x + f0 * a3.x + f1 * a3.y, fm * a0.y + f2 * a2.y + f0 * a3.y - f1 * a3.x);
+            const C h1 = mk<C>(fm * a1.x + f0 * a2.x - f1 * a2.y - f2 * a3.x, fm * a1.y + f0 * a2.y + f1 * a2.x - f2 * a3.y);
+            const C h2 = mk<C>(f2 * a0.x + f0 * a1.x + f1 * a1.y - fm * a2.x, f2 * a0.y + f0 * a1.y - f1 * a1.x - fm * a2.y);
+            const C h3 = mk<C>(f0 * a0.x - f1 * a0.y - f2 * a1.x - fm * a3.x, f0 * a0.y + f1 * a0.x - f2 * a1.y - fm * a3.y);
+            y[0][i] = mk<C>(fc * a0.x + h0.y, fc * a0.y - h0.x);
+            y[1][i] = mk<C>(fc * a1.x + h1.y, fc * a1.y - h1.x);
+            y[2][i] = mk<C>(fc * a2.x + h2.y, fc * a2.y - h2.x);
+            y[3][i] = mk<C>(fc * a3.x + h3.y, fc * a3.y - h3.x);
+        }
+    }
+#pragma unroll
+    for (int c2 = 0; c2 < CC; ++c2)
+#pragma unroll
+        for (int i = 0; i < PP; ++i) line0[c2 * comp_pitch + 17 * u + c * PP + i] = y[c2][i];
+    __syncwarp();
+#pragma unroll
+    for (int q = 0; q < 16; ++q) x[q] = me[q];
+}
+
 template <typename T, int N, int SMODE>
 __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const __grid_constant__ CUtensorMap tmap) {
     using C = typename CxOf<T>::type;
     constexpr int U = N / 16;
-    constexpr int CC = SMODE == SMODE_KD2 ? 2 : (SMODE == SMODE_KD4 ? 4 : 1);
+    constexpr int CC = (SMODE == SMODE_KD2 || SMODE == SMODE_KD2F) ? 2 : ((SMODE == SMODE_KD4 || SMODE == SMODE_KD4F) ? 4 : 1);
+    constexpr bool KTABLE = SMODE == SMODE_KD2 || SMODE == SMODE_KD4;
     constexpr int LAST = Sched<N>::M - 1;
     constexpr int TWN = Sched<N>::twoff(LAST);
     constexpr int TWP = (TWN + 7) & ~7;
+    // the pointwise table along the line (Schroedinger phase or Dirac momenta) sits in shared memory: with nearly all
+    // of it given to tiles, the L1 left over is too small to keep even a 2 KB table resident
+    constexpr int LTB = sring_line_table_bytes(SMODE, N, (int)sizeof(C));
     extern __shared__ __align__(128) unsigned char smem_raw[];
     C *stw = reinterpret_cast<C *>(smem_raw);
-    C *bufs = stw + TWP;
-    unsigned long long *full = reinterpret_cast<unsigned long long *>(bufs + (size_t)a.NB * a.bufstride);
-    volatile int *ktile = reinterpret_cast<volatile int *>(full + a.NB);  // as in ring_kernel
+    unsigned char *ltab = smem_raw + TWP * sizeof(C);
+    C *bufs = reinterpret_cast<C *>(ltab + LTB);
+    TileRing ring(bufs + (size_t)a.NB * a.bufstride, a.NB, a.G);
 
-    const int TL = a.TL, GT = a.GT, G = a.G, NB = a.NB;
+    const int TL = a.TL, GT = a.GT, G = a.G;
     const int grp = threadIdx.x / GT;
     const int tid = threadIdx.x - grp * GT;
-    // lane = u * TL + t within a component: exchanges confined to 32 / TL consecutive u stay inside a warp
-    const int gb = (G > 1 ? ((grp + 1) | (GT << 8)) : 0) | ((32 % TL == 0 && (U * TL) % 32 == 0) ? (GB_LANES_ARE_U | ((31 - __clz(TL)) << GB_TL_SHIFT)) : 0);
+    // thread layout (file header): t fastest, then UL consecutive u, then the component, then the rest of u
+    const int UL = TL >= 8 ? 1 : 8 / TL;
     const int t = tid % TL;
-    const int cu = tid / TL;
-    const int u = cu % U;
-    const int c = cu / U;
+    int r = tid / TL;
+    const int ulo = r % UL;
+    r /= UL;
+    const int c = r % CC;
+    const int u = ulo + UL * (r / CC);
+    // a warp holds 32 / (TL CC) consecutive u of TL lines: exchanges confined to that many u stay inside it
+    const int wl = TL * CC;
+    const int gb = (G > 1 ? ((grp + 1) | (GT << 8)) : 0) | ((32 % wl == 0 && GT % 32 == 0) ? (GB_LANES_ARE_U | ((31 - __clz(wl)) << GB_TL_SHIFT)) : 0);
     const unsigned tile_bytes = (unsigned)(CC * TL * N * sizeof(C));
     const int nloc = a.ntiles > (int)blockIdx.x ? (a.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const int nbox = N / a.box_rows;
@@ -55,19 +156,15 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
         const int tile = tile_of(k);
         const int o = tile / a.tiles_per_outer, i0 = (tile % a.tiles_per_outer) * TL;
         C *dst = bufs + (size_t)b * a.bufstride;
-        mbar_expect_tx(&full[b], tile_bytes);
+        mbar_expect_tx(ring.full(b), tile_bytes);
         for (int cc = 0; cc < CC; ++cc)
             for (int j = 0; j < nbox; ++j)
-                tma_load_3d(dst + (size_t)(cc * N + j * a.box_rows) * TL, &tmap, 2 * i0, j * a.box_rows, CC > 1 ? cc : o, &full[b]);
+                tma_load_3d(dst + (size_t)(cc * N + j * a.box_rows) * TL, &tmap, 2 * i0, j * a.box_rows, CC > 1 ? cc : o, ring.full(b));
     };
 
     // let the next pass of the stream start its own setup as SMs free up
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    if (threadIdx.x == 0) {
-        ktile[NB] = NB;
-        for (int b = 0; b < NB; ++b) mbar_init(&full[b], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
+    ring.init();
     {
         const C *__restrict__ gtw = reinterpret_cast<const C *>(a.tw);
         for (int i = threadIdx.x; i < TWN; i += blockDim.x) stw[i] = gtw[i];
@@ -75,26 +172,25 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
     __syncthreads();
     // everything above touched only plan-owned tables; psi is valid once the previous pass has completed
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    // every group owns NBG = NB / G buffers: its leader fills them, its threads consume them, so a buffer's
-    // mbarrier never sees a waiter that is not in step with its fills
-    const int NBG = NB / G;
-    auto refill = [&](int kn, int b) {
-        if (kn < nloc) {
-            ktile[b] = kn;
-            issue(kn, b);
-        } else {
-            ktile[b] = -1;
-            mbar_arrive(&full[b]);
-        }
+    auto refill = [&](int k, int b) {
+        ring.mark(b, k, nloc);
+        if (k < nloc) issue(k, b);
     };
     if (tid == 0)
-        for (int j = 0; j < NBG; ++j) refill(grp * NBG + j, grp * NBG + j);
+        for (int j = 0; j < ring.owned(grp); ++j) refill(grp + G * j, grp + G * j);
+    if constexpr (LTB > 0) {
+        // (the line table may have been rebuilt for this step by the kernel before this one, hence after the wait)
+        const double *__restrict__ src = reinterpret_cast<const double *>(SMODE == SMODE_KS ? a.kph0 : (const void *)a.kcp0);
+        double *dst = reinterpret_cast<double *>(ltab);
+        constexpr int ND = (SMODE == SMODE_KS ? N * (int)sizeof(C) : N * 8) / 8;
+        for (int i = threadIdx.x; i < ND; i += blockDim.x) dst[i] = src[i];
+        __syncthreads();
+    }
 
     for (int j = 0;; ++j) {
-        const int b = grp * NBG + j % NBG;
-        mbar_wait(&full[b], (unsigned)((j / NBG) & 1));
-        const int k = ktile[b];
+        const int k = ring.wait(grp, j);
         if (k < 0) break;
+        const int b = ring.buffer(grp, j);
         C *buf = bufs + (size_t)b * a.bufstride;
         C *dense = buf + (size_t)c * N * TL + t;     // TMA layout [CC][N][TL]: row r of this line at dense[r * TL]
         C *sl = buf + (c * TL + t) * a.pitch;        // exchange layout: padded lines
@@ -112,10 +208,26 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
 
         gsync(gb);  // the exchange layout overlaps the TMA layout of other warps' lines
 
-        if constexpr (SMODE != SMODE_DIT) DifChain<T, N, 0, -1>::run(x, u, stw, sl, gb);
+        [[maybe_unused]] DiracScalars<(CC > 1 ? CC : 2)> dks;
+        [[maybe_unused]] double w1 = 0.0, w2 = 0.0;  // c pi_1, c pi_2 of this line (pi = k - q Abar_n, reading G16)
+        [[maybe_unused]] const double mc2 = a.mass * a.clight * a.clight;
+        if constexpr (CC > 1) {
+            if (a.ndim == 2) w1 = a.clight * (a.kv2[line % a.rest1] - a.sh[1]);
+            if (a.ndim == 3) {
+                w1 = a.clight * (a.kv1[line / a.rest1] - a.sh[1]);
+                w2 = a.clight * (a.kv2[line % a.rest1] - a.sh[2]);
+            }
+        }
+        if constexpr (SMODE == SMODE_DIT) {
+        } else if constexpr (CC > 1 && !KTABLE) {
+            const double r12 = w1 * w1 + w2 * w2 + mc2 * mc2;
+            DifChain<T, N, 0, -1>::run(x, u, stw, sl, gb, [&]() { dirac_scalars<CC, U>(dks, u, c, reinterpret_cast<const double *>(ltab), r12, a.dt, a.scale); });
+        } else {
+            DifChain<T, N, 0, -1>::run(x, u, stw, sl, gb);
+        }
 
         if constexpr (SMODE == SMODE_KS) {
-            const C *__restrict__ k0 = reinterpret_cast<const C *>(a.kph0);
+            const C *k0 = reinterpret_cast<const C *>(ltab);
             C s = mk<C>((T)1, (T)0);
             bool has_s = false;
             if (a.kph1) {
@@ -133,24 +245,18 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
                 if (has_s) f = cmul(f, s);
                 x[q] = cmul(x[q], f);
             }
-        } else if constexpr (SMODE == SMODE_KD2 || SMODE == SMODE_KD4) {
-            double p1 = 0.0, p2 = 0.0;
-            if (a.ndim == 2) p1 = a.kv2[line % a.rest1] - a.sh[1];
-            if (a.ndim == 3) {
-                p1 = a.kv1[line / a.rest1] - a.sh[1];
-                p2 = a.kv2[line % a.rest1] - a.sh[2];
-            }
-            dirac_kinetic<T, CC, U>(x, u, c, sl, buf + t * a.pitch, TL * a.pitch, gb, a.kv0, a.sh[0], p1, p2, a.mass, a.clight, a.dt, a.scale);
+        } else if constexpr (CC > 1) {
+            dirac_kinetic_warp<T, CC, U, KTABLE>(x, u, c, sl + 17 * u, buf + t * a.pitch, TL * a.pitch, reinterpret_cast<const double *>(ltab), w1, w2, mc2,
+                                                 dks, reinterpret_cast<const double2 *>(a.ktab) + line, a.inner);
         }
 
         if constexpr (SMODE != SMODE_DIF) DitChain<T, N, LAST, +1>::run(x, u, stw, sl, gb);
 
         fence_async_smem();  // generic-proxy accesses of the buffer before its refill through the async proxy
-        gsync(gb);  // every thread of the group is done with the exchange layout
+        gsync(gb);           // every thread of the group is done with the exchange layout
+        // refill the buffer at once and store from registers (a warp instruction writes 32/TL rows of TL complex numbers)
+        if (tid == 0) refill(ring.claim(), b);
         {
-            // store from registers (a warp instruction writes 32/TL rows of TL complex numbers) and refill the
-            // buffer at once
-            if (tid == 0) refill(atomicAdd(const_cast<int *>(&ktile[NB]), 1), b);
             const long long o = tile / a.tiles_per_outer;
             const long long i0 = (long long)(tile % a.tiles_per_outer) * TL;
             C *gout = reinterpret_cast<C *>(a.psi) + (CC > 1 ? (long long)c * a.comp_stride : o * (long long)N * a.inner) + i0 + t;

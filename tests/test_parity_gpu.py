@@ -180,7 +180,7 @@ def test_schroedinger_with_vector_potential(torch):
 # ---------------------------------------------------------------------------------------------------------
 # every pipeline variant computes the same step: direct kernel, forced/disabled TMA ring, group and buffer counts
 # ---------------------------------------------------------------------------------------------------------
-OPT_TL_STRIDED, OPT_GROUPS, OPT_RING, OPT_THREADS, OPT_SRING = 2, 4, 5, 6, 7
+OPT_TL_STRIDED, OPT_GROUPS, OPT_RING, OPT_THREADS, OPT_SRING, OPT_DIRAC_TABLE = 2, 4, 5, 6, 7, 8
 VARIANTS = [
     ("direct_strided", [(OPT_SRING, 2)]),
     ("ring_forced", [(OPT_SRING, 1)]),
@@ -190,6 +190,9 @@ VARIANTS = [
     ("three_buffers", [(OPT_GROUPS, 2), (OPT_RING, 3)]),
     ("cta384", [(OPT_THREADS, 384)]),
     ("cta512", [(OPT_THREADS, 512)]),
+    ("dirac_table", [(OPT_DIRAC_TABLE, 1)]),
+    ("rows64B_one_spare_buffer", [(OPT_TL_STRIDED, 4), (OPT_GROUPS, 1), (OPT_RING, 2)]),
+    ("many_buffers_one_group", [(OPT_GROUPS, 1), (OPT_RING, 6)]),
 ]
 
 
