@@ -66,6 +66,9 @@ def lib():
         L.orc_dirac_u.argtypes = [ctypes.c_int, ctypes.c_int, dp, ctypes.c_double, ctypes.c_double, dp]
         L.orc_step.argtypes = [ctypes.POINTER(_Params), dp, dp, dp, ctypes.c_int64, ctypes.c_int64]
         L.orc_step.restype = ctypes.c_int
+        L.orc_step_apos.argtypes = [ctypes.POINTER(_Params), dp, dp, dp, dp, ctypes.c_int64, ctypes.c_int64]
+        L.orc_step_apos.restype = ctypes.c_int
+        L.orc_alpha_rotation.argtypes = [ctypes.c_int, ctypes.c_int, dp, dp]
         L.orc_norm.argtypes = [ctypes.POINTER(_Params), dp]
         L.orc_norm.restype = ctypes.c_double
         L.orc_inverse_sample.argtypes = [ctypes.POINTER(_Params), dp, dp, dp, ctypes.c_int64, dp]
@@ -123,6 +126,14 @@ def dirac_u(ncomp: int, p, mass: float, c: float) -> np.ndarray:
     return u
 
 
+def alpha_rotation(ncomp: int, a) -> np.ndarray:
+    """exp(i sum_i a_i alpha_i) in the closed form of eq. 23/24, as the oracle evaluates it."""
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    M = np.zeros((ncomp, ncomp), dtype=np.complex128)
+    lib().orc_alpha_rotation(ncomp, a.size, _dp(a), _dp(M))
+    return M
+
+
 class Solver:
     """The oracle's view of one problem: grid, constants, potential, field table."""
 
@@ -143,6 +154,7 @@ class Solver:
         self.p.nvals = 0
         self.V = None
         self.step_avg = None
+        self.A_pos = None
         self.time_index = 0
 
     def set_potential(self, V):
@@ -156,6 +168,10 @@ class Solver:
             self.step_avg = np.ascontiguousarray(step_avg, dtype=np.float64).reshape(-1, len(self.sizes)).copy()
             self.p.nvals = self.step_avg.shape[0]
 
+    def set_vector_potential(self, A):
+        """Step-averaged position-dependent A(r), shape (ndim, *sizes), applied in position space (eq. 26); None = off."""
+        self.A_pos = None if A is None else np.ascontiguousarray(A, dtype=np.float64).reshape((len(self.sizes),) + self.sizes).copy()
+
     def set_time_index(self, n):
         self.time_index = int(n)
 
@@ -163,7 +179,12 @@ class Solver:
         """Returns a new array; psi has shape (ncomp, *sizes) or sizes when ncomp == 1."""
         out = np.ascontiguousarray(psi, dtype=np.complex128).copy()
         assert out.size == self.p.ncomp * int(np.prod(self.sizes))
-        rc = lib().orc_step(ctypes.byref(self.p), _dp(out), _dp(self.V), _dp(self.step_avg), self.time_index, int(nsteps))
+        if self.A_pos is not None:
+            rc = lib().orc_step_apos(ctypes.byref(self.p), _dp(out), _dp(self.V), _dp(self.step_avg), _dp(self.A_pos), self.time_index, int(nsteps))
+            if rc == -2:
+                raise ValueError("oracle: the position-space vector potential needs a Dirac spinor (ncomp 2 or 4)")
+        else:
+            rc = lib().orc_step(ctypes.byref(self.p), _dp(out), _dp(self.V), _dp(self.step_avg), self.time_index, int(nsteps))
         if rc != 0:
             raise ValueError("oracle: field table shorter than the steps requested")
         self.time_index += int(nsteps)

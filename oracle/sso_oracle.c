@@ -366,6 +366,94 @@ static void kinetic_step(const orc_params *P, cplx *psi, const double *Abar) {
 }
 
 /*
+ * Position-space vector-potential factor of the Dirac equation (the paper's own treatment of A(x,t)):
+ * the split of PAPER.md:138-144 (eq. 18a) puts c sum_i alpha_i (-q A_i(x,t)) into A_1, next to q phi; the two
+ * parts commute (eq. 19-22), and the exponential of the matrix part is, by the algebra of the
+ * alpha_i (eq. 23/24),
+ *     exp(i sum_i a_i alpha_i) = cos(a) + i (sum_i a_i alpha_i / a) sin(a),   a = sqrt(sum_i a_i^2),
+ * here with a_i = delta * q * c * Abar_i(r), Abar_i = tau * (step average of A_i at r) the time integral of
+ * eq. 25a.  For q = -1 this is eq. 26 as printed (reading G4); in one dimension it is
+ * eq. 34.  Aavg: [ndim][N] step averages of A on the lattice.  a = 0 leaves psi unchanged.
+ */
+static void position_rotation(const orc_params *P, cplx *psi, const double *Aavg, double delta) {
+    int64_t N = 1;
+    for (int a = 0; a < P->ndim; ++a) N *= P->n[a];
+    int C = P->ncomp;
+    cplx al[3 * 4 * 4], be[4 * 4];
+    dirac_matrices(C, al, be);
+    double coef = delta * P->charge * P->c * P->dt;
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < N; ++j) {
+        double ai[3] = {0, 0, 0}, a2 = 0.0;
+        for (int a = 0; a < P->ndim; ++a) {
+            ai[a] = coef * Aavg[(int64_t)a * N + j];
+            a2 += ai[a] * ai[a];
+        }
+        double an = sqrt(a2);
+        if (an == 0.0) continue;
+        cplx M[16], in[4], out[4];
+        for (int r = 0; r < C; ++r)
+            for (int s = 0; s < C; ++s) {
+                cplx acc = (r == s) ? cos(an) : 0.0;
+                for (int a = 0; a < P->ndim; ++a) acc += I * (ai[a] / an) * sin(an) * al[(a * C + r) * C + s];
+                M[r * C + s] = acc;
+            }
+        for (int s = 0; s < C; ++s) in[s] = psi[(int64_t)s * N + j];
+        for (int r = 0; r < C; ++r) {
+            cplx acc = 0.0;
+            for (int s = 0; s < C; ++s) acc += M[r * C + s] * in[s];
+            out[r] = acc;
+        }
+        for (int r = 0; r < C; ++r) psi[(int64_t)r * N + j] = out[r];
+    }
+}
+
+/* the matrix of the factor above for one point, for the pins: a_i given directly */
+void orc_alpha_rotation(int ncomp, int ndim, const double *ai, double *M_ri) {
+    int C = ncomp;
+    cplx *M = (cplx *)M_ri;
+    cplx al[3 * 4 * 4], be[4 * 4];
+    dirac_matrices(C, al, be);
+    double a2 = 0.0;
+    for (int a = 0; a < ndim; ++a) a2 += ai[a] * ai[a];
+    double an = sqrt(a2);
+    for (int r = 0; r < C; ++r)
+        for (int s = 0; s < C; ++s) {
+            cplx acc = (r == s) ? (an == 0.0 ? 1.0 : cos(an)) : 0.0;
+            if (an != 0.0)
+                for (int a = 0; a < ndim; ++a) acc += I * (ai[a] / an) * sin(an) * al[(a * C + r) * C + s];
+            M[r * C + s] = acc;
+        }
+}
+
+/*
+ * The step with the position-space factor: as orc_step, with U_A1(1/2) = [scalar phase] x [rotation above] on both
+ * sides of the Fourier sandwich (eq. 7 with the A_1 of eq. 18a; the two parts of A_1 commute, eq. 19-22).
+ * Aavg: [ndim][N] step average of the position-dependent A(r), the same for every step of the call.  Dirac only.
+ */
+int orc_step_apos(const orc_params *P, double *psi_ri, const double *V, const double *step_avg, const double *Aavg, int64_t n0step, int64_t nsteps) {
+    cplx *psi = (cplx *)psi_ri;
+    int64_t N = 1;
+    for (int a = 0; a < P->ndim; ++a) N *= P->n[a];
+    if (P->ncomp < 2 || Aavg == NULL) return -2;
+    if (P->field_kind != ORC_FIELD_NONE && (step_avg == NULL || n0step + nsteps > P->nvals)) return -1;
+    for (int64_t s = 0; s < nsteps; ++s) {
+        int64_t n = n0step + s;
+        const double *avg = (P->field_kind != ORC_FIELD_NONE) ? step_avg + n * P->ndim : NULL;
+        const double *Ebar = (P->field_kind == ORC_FIELD_E) ? avg : NULL;
+        const double *Abar = (P->field_kind == ORC_FIELD_A) ? avg : NULL;
+        potential_half_step(P, psi, V, Ebar);
+        position_rotation(P, psi, Aavg, 0.5);
+        for (int cpt = 0; cpt < P->ncomp; ++cpt) orc_fft((double *)(psi + (int64_t)cpt * N), P->ndim, P->n, -1);
+        kinetic_step(P, psi, Abar);
+        for (int cpt = 0; cpt < P->ncomp; ++cpt) orc_fft((double *)(psi + (int64_t)cpt * N), P->ndim, P->n, +1);
+        position_rotation(P, psi, Aavg, 0.5);
+        potential_half_step(P, psi, V, Ebar);
+    }
+    return 0;
+}
+
+/*
  * Advance psi ([ncomp][n0][n1][n2] C order, interleaved re/im doubles) by
  * nsteps steps starting at step index n0step.  V: real potential energy
  * q phi(r) on the grid or NULL.  step_avg: [nvals][ndim] averages of E or A

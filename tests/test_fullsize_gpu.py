@@ -47,6 +47,41 @@ def test_full_size_first_steps_and_samples(torch, name, make, prec, nsteps):
         assert np.abs(flat[:, i] - s).max() <= TOL[prec] * scale, (name, i)
 
 
+FULL100 = [
+    ("cfg2a", lambda: wl.config2(nsteps=100), sso.C128),
+    ("cfg2b", lambda: wl.config2(nsteps=100), sso.C64),
+    ("cfg4", lambda: wl.config4(nsteps=100), sso.C128),
+    ("cfg3", lambda: wl.config3(nsteps=100), sso.C128),
+    ("cfg5", lambda: wl.config5(nsteps=100), sso.C128),
+]
+
+
+@pytest.mark.parametrize("name,make,prec", FULL100, ids=[f[0] for f in FULL100])
+def test_full_size_100_steps(torch, name, make, prec):
+    """north_star's bar as stated: relative L2 error <= 1e-11 (complex128) / 2e-5 (complex64) after 100 steps, at
+    BASELINE.json's full sizes, default options (the launch configuration bench.py times), element-wise bound too.
+    The oracle needs about 4 / 2 / 16 / 110 s for configs 2 / 4 / 3 / 5 on 16 host cores."""
+    w = make()
+    got, nrm = gpu_steps(torch, w, 100, prec)
+    want = oracle_steps(w, 100, prec)
+    err = rel_l2(got.astype(np.complex128), want)
+    assert err <= TOL[prec], (name, err)
+    peak = np.abs(want).max()
+    assert np.abs(got - want).max() <= 5 * TOL[prec] * peak, name
+    assert abs(nrm - 1.0) < (1e-11 if prec == sso.C128 else 1e-4)
+
+
+@pytest.mark.parametrize("cfg,nsteps", [(2, 300), (3, 80), (5, 24)])
+def test_full_size_runs_are_bitwise_reproducible(torch, cfg, nsteps):
+    """Many tiles per ring buffer, many steps, twice: the two results must be bit-identical.  A buffer handed back to
+    the copy engine before every thread is done with it (the cross-proxy ordering the refill relies on) shows up as
+    run-to-run differences long before it shows up as a parity failure."""
+    w = wl.CONFIGS[cfg](nsteps=nsteps)
+    a, _ = gpu_steps(torch, w, nsteps)
+    b, _ = gpu_steps(torch, w, nsteps)
+    assert np.array_equal(a.view(np.float64), b.view(np.float64))
+
+
 @pytest.mark.parametrize("cfg,prec", [(2, sso.C128), (2, sso.C64), (3, sso.C128), (4, sso.C128), (5, sso.C128)])
 def test_full_size_unitarity_and_reversibility(torch, cfg, prec):
     """Strang step is unitary and symmetric: the norm stays 1 and stepping with -dt (fields replayed
@@ -138,6 +173,58 @@ def test_error_paths_on_device(torch):
     assert torch.equal(psi, before)  # failed calls touched nothing
     p.destroy()
     p.destroy()  # idempotent
+
+
+def test_binding_rejects_mismatched_buffers(torch):
+    """The C ABI takes bare pointers; the Python binding refuses buffers that do not match the plan."""
+    w = wl.config2(sizes=(32, 64), nsteps=2)
+    p = make_plan(w)
+    good = torch.from_numpy(w.psi0.copy()).cuda()
+    with pytest.raises(ValueError):
+        p.step(good.to(torch.complex64), 1)           # element width
+    with pytest.raises(ValueError):
+        p.step(good[:, :16], 1)                        # size
+    with pytest.raises(ValueError):
+        p.step(good.transpose(1, 2), 1)                # contiguity
+    with pytest.raises(ValueError):
+        p.step(torch.from_numpy(w.psi0.copy()), 1)     # host tensor for a device argument
+    with pytest.raises(ValueError):
+        p.step_host(good, 1)                           # device tensor for a host argument
+    with pytest.raises(ValueError):
+        p.set_potential(w.V.astype(np.float32))        # V must be float64
+    with pytest.raises(ValueError):
+        p.norm(good[:, :16])
+    p.step(good, 1)
+    p.destroy()
+
+
+def test_changing_the_potential_representation_invalidates_the_potential(torch):
+    w = wl.config2(sizes=(32, 64), nsteps=2)
+    p = make_plan(w)
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    p.set_option(sso.OPT_POTENTIAL_PHASE, 1)
+    with pytest.raises(sso.SsoError) as e:
+        p.step(psi, 1)
+    assert e.value.code == sso.ERR_STATE
+    p.set_potential(w.V)
+    p.step(psi, 2)
+    torch.cuda.synchronize()
+    assert rel_l2(psi.cpu().numpy(), oracle_steps(w, 2)) < 1e-13
+    p.destroy()
+
+
+def test_profile_step_reports_every_pass(torch):
+    w = wl.config3(sizes=(32, 32, 64), nsteps=4)
+    p = make_plan(w)
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    rows = p.profile_step(psi, 4)
+    torch.cuda.synchronize()
+    names = {r[0].split(" [")[0]: r[1] for r in rows}
+    assert names["opening"] == 1 and names["closing"] == 1 and names["potential"] == 3 and names["kinetic"] == 4
+    assert sum(r[1] for r in rows if r[0].startswith("middle axis")) == 8
+    assert all(r[2] > 0.0 for r in rows)
+    assert rel_l2(psi.cpu().numpy(), oracle_steps(w, 4)) < 1e-13  # the profiled call is a real step
+    p.destroy()
 
 
 def test_potential_sources_agree(torch):
