@@ -118,6 +118,23 @@ int sso_set_potential(sso_plan *plan, const double *V, int on_device, void *stre
  */
 int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nvals);
 
+/*
+ * Position-dependent vector potential A(r) of a Dirac plan, applied in POSITION space as the paper does
+ * (eq. 18a: c sum_i alpha_i (-q A_i(x,t)) belongs to A_1, next to q phi):  both potential half
+ * steps of a step also multiply every spinor by
+ *     exp(i sum_i a_i alpha_i) = cos a + i (sum_i a_i alpha_i / a) sin a,   a_i = (tau/2) q c A_i(r),  a = |a|
+ * (eq. 23/24; with q = -1 this is eq. 26 as printed; eq. 34, in
+ * one dimension).  A is the STEP AVERAGE of the field on the lattice (its time integral over a step divided by
+ * tau, reading G12), double[ndim][n0][n1][n2] in C order, host or device pointer; copied, the caller keeps
+ * ownership; it is used for every following step until replaced (a time-dependent A(r,t) is set step by step);
+ * NULL switches the factor off.  Independent of SSO_FIELD_A, whose homogeneous A(t) enters the kinetic factor
+ * (reading G16); the two splittings agree to O(tau^2).  ncomp = 1 gives SSO_ERR_UNSUPPORTED.  In this version the
+ * factor runs as a kernel of its own where psi is in position space on every axis, i.e. before the first and after
+ * the last pass of a step: while it is set, consecutive half steps are not merged (a 2D step costs an opening, a
+ * kinetic and a closing pass plus two rotation kernels).  Synchronises `stream`.
+ */
+int sso_set_vector_potential(sso_plan *plan, const double *A, int on_device, void *stream);
+
 /* Step counter n used to index step_avg (t_n = n dt, reading G21); sso_step advances it. */
 int sso_set_time_index(sso_plan *plan, int64_t n);
 int sso_get_time_index(const sso_plan *plan, int64_t *n);
@@ -170,7 +187,8 @@ int sso_launch_count(const sso_plan *plan, int64_t nsteps, int64_t *count);
 #define SSO_PASS_MIDDLE_INVERSE 5 /* 3D: inverse transform along the middle axis                   */
 #define SSO_PASS_LINE_1D 6        /* 1D: every step of the call in one persistent launch           */
 #define SSO_PASS_TABLES 7         /* small per-step table kernels (field phases, kinetic phases)   */
-#define SSO_PASS_KINDS 8
+#define SSO_PASS_ROTATION 8       /* position-space vector-potential factor (sso_set_vector_potential) */
+#define SSO_PASS_KINDS 9
 int sso_profile_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream, int64_t *count, double *mean_us);
 const char *sso_pass_name(int kind);
 

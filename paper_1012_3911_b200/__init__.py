@@ -28,8 +28,9 @@ SYMBOLS = (
     "sso_plan_create", "sso_set_constants", "sso_set_potential", "sso_set_field", "sso_set_time_index",
     "sso_get_time_index", "sso_step", "sso_step_host", "sso_norm", "sso_set_option", "sso_launch_count",
     "sso_destroy", "sso_last_error", "sso_version", "sso_debug_layout", "sso_profile_step", "sso_pass_name",
+    "sso_set_vector_potential",
 )
-PASS_KINDS = 8
+PASS_KINDS = 9
 
 
 class SsoError(RuntimeError):
@@ -53,6 +54,7 @@ def lib() -> ctypes.CDLL:
         L.sso_set_constants.argtypes = [vp, dbl, dbl, dbl]
         L.sso_set_potential.argtypes = [vp, vp, ci, vp]
         L.sso_set_field.argtypes = [vp, ci, vp, i64]
+        L.sso_set_vector_potential.argtypes = [vp, vp, ci, vp]
         L.sso_set_time_index.argtypes = [vp, i64]
         L.sso_get_time_index.argtypes = [vp, ctypes.POINTER(i64)]
         L.sso_step.argtypes = [vp, vp, i64, vp]
@@ -163,6 +165,11 @@ class Plan:
         nvals = step_avg.shape[0]
         _check_buffer(step_avg, nvals * len(self.sizes) * 8, 8, False, "step_avg")
         self._ck(lib().sso_set_field(self._h, int(kind), _ptr(step_avg), int(nvals)))
+
+    def set_vector_potential(self, A, on_device: bool = False, stream=None) -> None:
+        """A: float64 step-averaged A(r), shape (ndim, *sizes) (numpy on host, or a torch CUDA tensor); None = off."""
+        _check_buffer(A, self._npts * len(self.sizes) * 8, 8, bool(on_device), "A")
+        self._ck(lib().sso_set_vector_potential(self._h, _ptr(A), int(bool(on_device)), _stream(stream)))
 
     def set_time_index(self, n: int) -> None:
         self._ck(lib().sso_set_time_index(self._h, int(n)))

@@ -142,6 +142,48 @@ template <typename T> __global__ void build_erows_kernel(const ERowsArgs e) {
     }
 }
 
+// Position-space vector-potential factor of the Dirac step (eq. 18a; 168-184 eq. 23/24; 188-198
+// eq. 25/26; 236 eq. 34): at every lattice point  psi <- (cos a + i (sum_i a_i alpha_i / a) sin a) psi,
+// a_i = coef * A_i(r), coef = delta tau q c, a = |a|.  With the Dirac representation (eq. 16)
+// sum_i a_i alpha_i = [[0, sigma.a], [sigma.a, 0]]; the two-component forms are its {1,4} block (eq. 17, reading G7).
+// One thread per point holds all components; streaming, one read and one write of psi.
+template <typename T, int CC>
+__global__ void apos_rotate_kernel(void *__restrict__ psi_, const double *__restrict__ A, long long npts, int ndim, double coef) {
+    using C = typename Cx2<T>::type;
+    C *psi = reinterpret_cast<C *>(psi_);
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < npts; j += (long long)gridDim.x * blockDim.x) {
+        const double a1 = coef * A[j];
+        const double a2 = ndim > 1 ? coef * A[npts + j] : 0.0;
+        const double a3 = ndim > 2 ? coef * A[2 * npts + j] : 0.0;
+        const double an = sqrt(a1 * a1 + a2 * a2 + a3 * a3);
+        if (an == 0.0) continue;
+        double sn, cs;
+        sincos(an, &sn, &cs);
+        const double s = sn / an;
+        const T fc = (T)cs, f1 = (T)(s * a1), f2 = (T)(s * a2), f3 = (T)(s * a3);
+        // i (x + i y) = -y + i x
+        if (CC == 2) {
+            const C p0 = psi[j], p1 = psi[npts + j];
+            // (a1 - i a2) p1 and (a1 + i a2) p0
+            const T h0x = f1 * p1.x + f2 * p1.y, h0y = f1 * p1.y - f2 * p1.x;
+            const T h1x = f1 * p0.x - f2 * p0.y, h1y = f1 * p0.y + f2 * p0.x;
+            psi[j] = C{fc * p0.x - h0y, fc * p0.y + h0x};
+            psi[npts + j] = C{fc * p1.x - h1y, fc * p1.y + h1x};
+        } else {
+            const C u0 = psi[j], u1 = psi[npts + j], l0 = psi[2 * npts + j], l1 = psi[3 * npts + j];
+            // sigma.a (v0, v1) = (a3 v0 + (a1 - i a2) v1, (a1 + i a2) v0 - a3 v1)
+            const T g0x = f3 * l0.x + f1 * l1.x + f2 * l1.y, g0y = f3 * l0.y + f1 * l1.y - f2 * l1.x;  // (sigma.a l)_0
+            const T g1x = f1 * l0.x - f2 * l0.y - f3 * l1.x, g1y = f1 * l0.y + f2 * l0.x - f3 * l1.y;  // (sigma.a l)_1
+            const T k0x = f3 * u0.x + f1 * u1.x + f2 * u1.y, k0y = f3 * u0.y + f1 * u1.y - f2 * u1.x;  // (sigma.a u)_0
+            const T k1x = f1 * u0.x - f2 * u0.y - f3 * u1.x, k1y = f1 * u0.y + f2 * u0.x - f3 * u1.y;  // (sigma.a u)_1
+            psi[j] = C{fc * u0.x - g0y, fc * u0.y + g0x};
+            psi[npts + j] = C{fc * u1.x - g1y, fc * u1.y + g1x};
+            psi[2 * npts + j] = C{fc * l0.x - k0y, fc * l0.y + k0x};
+            psi[3 * npts + j] = C{fc * l1.x - k1y, fc * l1.y + k1x};
+        }
+    }
+}
+
 // norm: partial sums of |psi|^2 in double, warp-shuffle tree, fixed order (deterministic)
 template <typename T>
 __global__ void norm_partial_kernel(const void *__restrict__ psi, long long count, double *__restrict__ partial) {
@@ -297,6 +339,7 @@ struct sso_plan {
     int tmap_tl[3] = {0, 0, 0};
     int vrep = VREP_TABLE;
     bool kph_valid = false;
+    double *d_apos = nullptr; // step-averaged position-dependent A(r), [ndim][npts], or NULL (sso_set_vector_potential)
     void *d_ktab = nullptr;   // Dirac kinetic scalars per k point (SSO_OPT_DIRAC_TABLE = 1), else NULL
     double *d_kcp0 = nullptr; // Dirac: c (k_0 - q Abar_0) per slot of axis 0
     bool ktab_valid = false;  // both tables are current (plans without SSO_FIELD_A only; with it they change every step)
@@ -544,6 +587,7 @@ int sso_destroy(sso_plan *plan) {
     cudaFree(plan->d_vfull);
     cudaFree(plan->d_ktab);
     cudaFree(plan->d_kcp0);
+    cudaFree(plan->d_apos);
     for (int a = 0; a < 3; ++a) cudaFree(plan->d_erow[a]);
     cudaFree(plan->d_partial);
     cudaFree(plan->d_norm);
@@ -607,6 +651,26 @@ int sso_set_potential(sso_plan *plan, const double *V, int on_device, void *stre
     cudaFree(tmp);
     if (e != cudaSuccess) return cuda_fail(plan, e, "potential table kernel");
     plan->v_valid = true;
+    return SSO_OK;
+}
+
+int sso_set_vector_potential(sso_plan *plan, const double *A, int on_device, void *stream) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (plan->ncomp == 1)
+        return fail(plan, SSO_ERR_UNSUPPORTED, "the position-space vector potential is the Dirac interaction factor (ncomp 2 or 4)");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!A) {
+        cudaFree(plan->d_apos);
+        plan->d_apos = nullptr;
+        return SSO_OK;
+    }
+    const size_t bytes = sizeof(double) * (size_t)plan->npts * plan->ndim;
+    if (!plan->d_apos) {
+        cudaError_t e = cudaMalloc((void **)&plan->d_apos, bytes);
+        if (e != cudaSuccess) return fail(plan, SSO_ERR_ALLOC, std::string("vector potential: ") + cudaGetErrorString(e));
+    }
+    CK(cudaMemcpyAsync(plan->d_apos, A, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
     return SSO_OK;
 }
 
@@ -1174,6 +1238,22 @@ long long erow_chunk(const sso_plan *p) {
     return c < 1 ? 1 : c;
 }
 
+// position-space vector-potential factor over `delta` of a step (1/2: half step, 1: two merged half steps)
+int launch_rotation(sso_plan *plan, void *psi, double delta, cudaStream_t st) {
+    if (!plan->d_apos) return SSO_OK;
+    PassTimer timer(plan, SSO_PASS_ROTATION, st);
+    const double coef = delta * plan->dt * plan->charge * plan->clight;
+    const int blocks = plan->num_sms * 8;
+    if (plan->precision == SSO_C128) {
+        if (plan->ncomp == 2) apos_rotate_kernel<double, 2><<<blocks, 256, 0, st>>>(psi, plan->d_apos, plan->npts, plan->ndim, coef);
+        else apos_rotate_kernel<double, 4><<<blocks, 256, 0, st>>>(psi, plan->d_apos, plan->npts, plan->ndim, coef);
+    } else {
+        if (plan->ncomp == 2) apos_rotate_kernel<float, 2><<<blocks, 256, 0, st>>>(psi, plan->d_apos, plan->npts, plan->ndim, coef);
+        else apos_rotate_kernel<float, 4><<<blocks, 256, 0, st>>>(psi, plan->d_apos, plan->npts, plan->ndim, coef);
+    }
+    return pass_status(plan, "vector-potential rotation kernel", cudaGetLastError());
+}
+
 // (re)build the Schroedinger kinetic phase tables; with SSO_FIELD_A they depend on the step
 int build_kphase(sso_plan *plan, long long n, cudaStream_t st) {
     const bool shifted = plan->field_kind == SSO_FIELD_A;
@@ -1233,10 +1313,11 @@ long long launches_for(const sso_plan *p, long long nsteps) {
     const bool kshift = p->ncomp == 1 && p->field_kind == SSO_FIELD_A;
     const bool kbuild = p->ncomp == 1 && (kshift || !p->kph_valid);
     if (p->ndim == 1) {
+        if (p->d_apos) return nsteps * 3;  // rotation, one step, rotation
         if (kshift) return nsteps * (1 + p->ndim);
         return 1 + (kbuild ? p->ndim : 0);
     }
-    const long long chunk = erow_chunk(p);
+    const long long chunk = p->d_apos ? 1 : erow_chunk(p);
     const long long nchunks = (nsteps + chunk - 1) / chunk;
     if (p->ncomp > 1 && sring_shape(p, 0, p->ncomp, false).ok) cnt += dirac_tables_per_step(p) ? nsteps : (p->ktab_valid ? 0 : 1);  // Dirac kinetic tables
     bool eph = false;
@@ -1244,6 +1325,7 @@ long long launches_for(const sso_plan *p, long long nsteps) {
     cnt += nchunks * (eph ? 2 : 1);              // opening pass (+ field phase rows)
     cnt += nsteps * (p->ndim == 3 ? 3 : 1);      // kinetic sandwich (+ middle-axis DIF and DIT)
     cnt += nsteps;                               // potential sandwiches and the closing pass
+    if (p->d_apos) cnt += 2 * nchunks;           // position-space rotations before every opening and after every closing pass
     if (kshift) cnt += nsteps * p->ndim;
     else if (kbuild) cnt += p->ndim;
     return cnt;
@@ -1277,8 +1359,10 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
     if (nd == 1) {
         // one persistent CTA: V/2, then nsteps x [F K F^-1, V (merged) or V/2 (last)]
         const bool kshift = plan->ncomp == 1 && plan->field_kind == SSO_FIELD_A;
-        const long long chunk = kshift ? 1 : nsteps;  // step-dependent kinetic tables force one launch per step
+        // step-dependent kinetic tables, or the position-space rotation between the steps, force one launch per step
+        const long long chunk = (kshift || plan->d_apos) ? 1 : nsteps;
         for (long long s = 0; s < nsteps; s += chunk) {
+            if ((rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
             if (plan->ncomp == 1 && (rc = build_kphase(plan, n0 + s, st)) != SSO_OK) return rc;
             if (chunk > 0x7fffffffLL) return fail(plan, SSO_ERR_INVALID, "nsteps too large");
             Line1dLaunchFn l1 = (plan->ncomp == 1 && plan->field_kind != SSO_FIELD_E) ? find_line1d(plan->precision, plan->ax[0].n) : nullptr;
@@ -1300,10 +1384,13 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
             }
             PassSpec ps{0, kpw, -1, 1, 1, 0, 1, 1, 1, (int)chunk, n0 + s};
             if ((rc = launch(plan, psi, ps, st)) != SSO_OK) return rc;
+            if ((rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
         }
     } else {
         // chunks that share one set of field phase rows; each chunk opens and closes with a half step
-        const long long chunk = erow_chunk(plan);
+        // Between the passes of a chunk psi is in momentum space along the last axis, so the position-space
+        // rotation can only run before an opening and after a closing pass: with it every step is its own chunk.
+        const long long chunk = plan->d_apos ? 1 : erow_chunk(plan);
         SRingShape shk = sring_shape(plan, 0, plan->ncomp == 1 ? 1 : plan->ncomp, false);
         SRingShape shm = nd == 3 ? sring_shape(plan, 1, 1, true) : SRingShape{};
         for (long long c0 = 0; c0 < nsteps; c0 += chunk) {
@@ -1311,6 +1398,7 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
             const long long nb = n0 + c0;
             if ((rc = build_erows(plan, nb, ns, st)) != SSO_OK) return rc;
             // opening: V/2 in natural order, forward transform along the last axis, natural frequency order out
+            if ((rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
             if ((rc = launch_ring_pass(plan, psi, MODE_OPEN, 0, st)) != SSO_OK) return rc;
             for (long long s = 0; s < ns; ++s) {
                 const long long n = nb + s;
@@ -1341,6 +1429,7 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
                 // F_last^-1 V(n, n+1) F_last, or the closing F_last^-1, V/2
                 if ((rc = launch_ring_pass(plan, psi, s + 1 < ns ? MODE_MID : MODE_CLOSE, s + 1, st)) != SSO_OK) return rc;
             }
+            if ((rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
         }
     }
     plan->tindex += nsteps;
@@ -1385,6 +1474,7 @@ const char *sso_pass_name(int kind) {
         case SSO_PASS_MIDDLE_INVERSE: return "middle axis [F_1^-1]";
         case SSO_PASS_LINE_1D: return "1D line, all steps in one launch";
         case SSO_PASS_TABLES: return "per-step tables";
+        case SSO_PASS_ROTATION: return "position-space vector-potential rotation";
     }
     return "";
 }

@@ -179,6 +179,46 @@ def test_random_state_3d_and_dirac(torch):
         assert rel_l2(got, want) <= 1e-13, (ncomp, sizes, rel_l2(got, want))
 
 
+def test_position_space_vector_potential(torch):
+    """The paper's own Dirac interaction factor (eq. 18a, 23-26, 34): A(r) applied in position space, merged between
+    steps, together with V, with and without a homogeneous A(t) in the kinetic factor, all lattice dimensions."""
+    cases = [(2, (256,), None), (4, (128,), wl.FIELD_A), (2, (64, 128), wl.FIELD_A), (4, (32, 64), None), (4, (16, 32, 32), None)]
+    for ncomp, sizes, kind in cases:
+        nd = len(sizes)
+        dx = (0.1,) * nd
+        rng = np.random.default_rng(100 * ncomp + nd)
+        psi0 = wl.random_state(sizes, ncomp, seed=5 * ncomp + nd, dx=dx)
+        R = wl.mesh(sizes, dx)
+        A = np.stack([40.0 * np.sin(0.7 * R[(a + 1) % nd] + a) + rng.uniform(-5, 5) for a in range(nd)])  # smooth, a.u.
+        w = wl.Workload("apos", sizes, dx, 1e-4, ncomp, 6, psi0, V=rng.uniform(-2000, 2000, size=sizes),
+                        field_kind=kind or wl.FIELD_NONE, step_avg=rng.uniform(-3, 3, size=(8, nd)) if kind else None)
+        for prec, tol in ((sso.C128, 1e-13), (sso.C64, 2e-6)):
+            p = make_plan(w, prec)
+            p.set_vector_potential(A)
+            s0 = psi0.astype(np.complex128 if prec == sso.C128 else np.complex64)
+            psi = torch.from_numpy(s0).cuda()
+            p.step(psi, 2)
+            p.step(psi, 4)
+            torch.cuda.synchronize()
+            o = make_oracle(w)
+            o.set_vector_potential(A)
+            want = o.step(s0.astype(np.complex128), 6)
+            err = rel_l2(psi.cpu().numpy().astype(np.complex128), want)
+            assert err <= tol, (ncomp, sizes, kind, prec, err)
+            assert p.launch_count(3) > 0
+            # switching the factor off again gives the plain step
+            p.set_vector_potential(None)
+            p.set_time_index(0)
+            psi = torch.from_numpy(s0).cuda()
+            p.step(psi, 2)
+            torch.cuda.synchronize()
+            assert rel_l2(psi.cpu().numpy().astype(np.complex128), oracle_steps(w, 2, psi0=s0)) <= tol
+            p.destroy()
+    with pytest.raises(sso.SsoError) as e:
+        sso.Plan((64,), (0.1,), 0.01, 1).set_vector_potential(np.ones((1, 64)))
+    assert e.value.code == sso.ERR_UNSUPPORTED
+
+
 def test_field_e_on_every_axis(torch):
     """Length-gauge field with components along all axes (the last axis uses the per-step line phase table)."""
     for sizes in ((64,), (32, 64), (16, 32, 64)):
