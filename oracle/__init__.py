@@ -74,6 +74,11 @@ def lib():
         L.orc_inverse_sample.argtypes = [ctypes.POINTER(_Params), dp, dp, dp, ctypes.c_int64, dp]
         L.orc_half_step_to_k.argtypes = [ctypes.POINTER(_Params), dp, dp, dp, ctypes.c_int64]
         L.orc_half_step_to_k.restype = ctypes.c_int
+        L.orc_overlap.argtypes = [ctypes.POINTER(_Params), dp, dp, dp]
+        L.orc_expect_r.argtypes = [ctypes.POINTER(_Params), dp, dp]
+        L.orc_expect_p.argtypes = [ctypes.POINTER(_Params), dp, dp]
+        L.orc_spectrum.argtypes = [dp, ctypes.c_int64, ctypes.c_double, dp, ctypes.c_int64, dp]
+        L.orc_filter_accumulate.argtypes = [ctypes.POINTER(_Params), dp, dp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double]
         _lib = L
     return _lib
 
@@ -132,6 +137,15 @@ def alpha_rotation(ncomp: int, a) -> np.ndarray:
     M = np.zeros((ncomp, ncomp), dtype=np.complex128)
     lib().orc_alpha_rotation(ncomp, a.size, _dp(a), _dp(M))
     return M
+
+
+def spectrum(chi, dts: float, E) -> np.ndarray:
+    """chi~(E) of eq. 41 from samples chi(n dts), n < len(chi), T = len(chi) dts."""
+    chi = np.ascontiguousarray(chi, dtype=np.complex128)
+    E = np.ascontiguousarray(E, dtype=np.float64)
+    out = np.zeros(E.size, dtype=np.complex128)
+    lib().orc_spectrum(_dp(chi), chi.size, float(dts), _dp(E), E.size, _dp(out))
+    return out
 
 
 class Solver:
@@ -210,3 +224,30 @@ class Solver:
             Ebar = np.ascontiguousarray(self.step_avg[n])
         lib().orc_inverse_sample(ctypes.byref(self.p), _dp(a), _dp(self.V), _dp(Ebar), int(flat_index), _dp(out))
         return out
+
+    # observables
+    def overlap(self, a: np.ndarray, b: np.ndarray) -> complex:
+        """<a|b> = sum conj(a) b prod dx  (chi(t) of eq. 40 with a = psi(0), b = psi(t))."""
+        a = np.ascontiguousarray(a, dtype=np.complex128)
+        b = np.ascontiguousarray(b, dtype=np.complex128)
+        out = np.zeros(2)
+        lib().orc_overlap(ctypes.byref(self.p), _dp(a), _dp(b), _dp(out))
+        return complex(out[0], out[1])
+
+    def expect_r(self, psi: np.ndarray) -> np.ndarray:
+        a = np.ascontiguousarray(psi, dtype=np.complex128)
+        out = np.zeros(len(self.sizes))
+        lib().orc_expect_r(ctypes.byref(self.p), _dp(a), _dp(out))
+        return out
+
+    def expect_p(self, psi: np.ndarray) -> np.ndarray:
+        a = np.ascontiguousarray(psi, dtype=np.complex128)
+        out = np.zeros(len(self.sizes))
+        lib().orc_expect_p(ctypes.byref(self.p), _dp(a), _dp(out))
+        return out
+
+    def filter_accumulate(self, acc: np.ndarray, psi: np.ndarray, t: float, T: float, E: float, dts: float) -> None:
+        """acc += psi (1 - cos(2 pi t/T)) exp(i E t) dts, in place (one term of eq. 42)."""
+        assert acc.dtype == np.complex128 and acc.flags.c_contiguous
+        a = np.ascontiguousarray(psi, dtype=np.complex128)
+        lib().orc_filter_accumulate(ctypes.byref(self.p), _dp(acc), _dp(a), float(t), float(T), float(E), float(dts))

@@ -35,6 +35,15 @@
  * 2..5 have no paper value to compare to: "parity unpinned beyond oracle +
  * invariants" for those.
  *
+ * Observables (end of file): overlap / autocorrelation
+ * chi(t) (eq. 40), <r>, <p>, windowed spectrum (eq. 41), eigenfunction filter
+ * (eq. 42), each the plain sum.  Pins (tests/test_oracle_observables.py):
+ * Gaussian-overlap closed form, plane-wave autocorrelation, packet centroid
+ * and momentum, Stoermer-Verlet kick, exact Hann-window identities, and the
+ * paper's soft-core ground-state energy -Z^2/2 for zeta = 1.4133 (1D) and
+ * 0.791 (2D) through the whole chi -> spectrum -> filter
+ * chain.
+ *
  * Units: atomic units, hbar = 1.
  */
 #include <complex.h>
@@ -551,4 +560,122 @@ int orc_half_step_to_k(const orc_params *P, double *psi_ri, const double *V, con
     for (int cpt = 0; cpt < P->ncomp; ++cpt) orc_fft((double *)(psi + (int64_t)cpt * N), P->ndim, P->n, -1);
     kinetic_step(P, psi, Abar);
     return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* Observables (section V.2).  New functions only:   */
+/* nothing above is changed.  All are the plain definitions, written   */
+/* as sums over the lattice (integrals -> sum * prod dx, reading G30). */
+/* Pins: tests/test_oracle_observables.py.                             */
+/* ------------------------------------------------------------------ */
+
+/* <a|b> = sum_c sum_r conj(a_c(r)) b_c(r) prod dx: the autocorrelation chi(t) of eq. 40
+ * with a = Psi(.,0), b = Psi(.,t).  out = (re, im). */
+void orc_overlap(const orc_params *P, const double *a_ri, const double *b_ri, double *out) {
+    const cplx *a = (const cplx *)a_ri, *b = (const cplx *)b_ri;
+    int64_t N = 1;
+    double vol = 1.0;
+    for (int ax = 0; ax < P->ndim; ++ax) {
+        N *= P->n[ax];
+        vol *= P->dx[ax];
+    }
+    int64_t M = N * P->ncomp;
+    double re = 0.0, im = 0.0;
+#pragma omp parallel for reduction(+ : re, im) schedule(static)
+    for (int64_t j = 0; j < M; ++j) {
+        cplx t = conj(a[j]) * b[j];
+        re += creal(t);
+        im += cimag(t);
+    }
+    out[0] = re * vol;
+    out[1] = im * vol;
+}
+
+/* <r_a> = sum_c sum_r r_a |psi_c(r)|^2 prod dx, a < ndim, on the grid r_j = (j - n/2) dx (G14) */
+void orc_expect_r(const orc_params *P, const double *psi_ri, double *out /*[ndim]*/) {
+    const cplx *psi = (const cplx *)psi_ri;
+    int64_t N = 1;
+    double vol = 1.0;
+    for (int ax = 0; ax < P->ndim; ++ax) {
+        N *= P->n[ax];
+        vol *= P->dx[ax];
+    }
+    for (int ax = 0; ax < P->ndim; ++ax) {
+        int64_t inner = 1;
+        for (int b = ax + 1; b < P->ndim; ++b) inner *= P->n[b];
+        double acc = 0.0;
+#pragma omp parallel for reduction(+ : acc) schedule(static)
+        for (int64_t j = 0; j < N; ++j) {
+            double r = r_of((j / inner) % P->n[ax], P->n[ax], P->dx[ax]);
+            double d = 0.0;
+            for (int cpt = 0; cpt < P->ncomp; ++cpt) {
+                cplx v = psi[(int64_t)cpt * N + j];
+                d += creal(v) * creal(v) + cimag(v) * cimag(v);
+            }
+            acc += r * d;
+        }
+        out[ax] = acc * vol;
+    }
+}
+
+/* <p_a> = sum_c sum_k k_a |psi~_c(k)|^2 prod dx / N  (canonical momentum, hbar = 1; psi~ = unnormalised forward DFT of
+ * eq. 12, so sum_k |psi~|^2 = N sum_r |psi|^2), k on the grid of G14 */
+void orc_expect_p(const orc_params *P, const double *psi_ri, double *out /*[ndim]*/) {
+    int64_t N = 1;
+    double vol = 1.0;
+    for (int ax = 0; ax < P->ndim; ++ax) {
+        N *= P->n[ax];
+        vol *= P->dx[ax];
+    }
+    cplx *w = (cplx *)malloc(sizeof(cplx) * (size_t)(N * P->ncomp));
+    memcpy(w, psi_ri, sizeof(cplx) * (size_t)(N * P->ncomp));
+    for (int cpt = 0; cpt < P->ncomp; ++cpt) orc_fft((double *)(w + (int64_t)cpt * N), P->ndim, P->n, -1);
+    for (int ax = 0; ax < P->ndim; ++ax) {
+        int64_t inner = 1;
+        for (int b = ax + 1; b < P->ndim; ++b) inner *= P->n[b];
+        double acc = 0.0;
+#pragma omp parallel for reduction(+ : acc) schedule(static)
+        for (int64_t j = 0; j < N; ++j) {
+            double k = k_of((j / inner) % P->n[ax], P->n[ax], P->dx[ax]);
+            double d = 0.0;
+            for (int cpt = 0; cpt < P->ncomp; ++cpt) {
+                cplx v = w[(int64_t)cpt * N + j];
+                d += creal(v) * creal(v) + cimag(v) * cimag(v);
+            }
+            acc += k * d;
+        }
+        out[ax] = acc * vol / (double)N;
+    }
+    free(w);
+}
+
+/* chi~(E) = int_0^T chi(t) (1 - cos(2 pi t/T)) exp(i t E) dt  (eq. 41) from samples chi(t_n),
+ * t_n = n dts, n < nt, T = nt dts, as the plain sum over samples times dts (reading G30; the window vanishes at both
+ * ends, so rectangle and trapezoid rule coincide).  chi_ri: [nt] complex; E: [nE]; out_ri: [nE] complex. */
+void orc_spectrum(const double *chi_ri, int64_t nt, double dts, const double *E, int64_t nE, double *out_ri) {
+    const cplx *chi = (const cplx *)chi_ri;
+    cplx *out = (cplx *)out_ri;
+    double T = (double)nt * dts;
+#pragma omp parallel for schedule(static)
+    for (int64_t e = 0; e < nE; ++e) {
+        cplx acc = 0.0;
+        for (int64_t n = 0; n < nt; ++n) {
+            double t = (double)n * dts;
+            double wdw = 1.0 - cos(2.0 * M_PI * t / T);
+            acc += chi[n] * wdw * (cos(t * E[e]) + I * sin(t * E[e]));
+        }
+        out[e] = acc * dts;
+    }
+}
+
+/* one term of eq. 42: acc(x) += Psi(x, t) (1 - cos(2 pi t/T)) exp(i E t) dts, every component */
+void orc_filter_accumulate(const orc_params *P, double *acc_ri, const double *psi_ri, double t, double T, double E, double dts) {
+    cplx *acc = (cplx *)acc_ri;
+    const cplx *psi = (const cplx *)psi_ri;
+    int64_t N = 1;
+    for (int ax = 0; ax < P->ndim; ++ax) N *= P->n[ax];
+    int64_t M = N * P->ncomp;
+    cplx wgt = (1.0 - cos(2.0 * M_PI * t / T)) * (cos(E * t) + I * sin(E * t)) * dts;
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < M; ++j) acc[j] += wgt * psi[j];
 }
