@@ -78,6 +78,9 @@ extern "C" {
 #define SSO_OPT_STRIDED_RING 7           /* strided-axis passes: 0 auto, 1 force the TMA ring, 2 direct kernel only */
 #define SSO_OPT_DIRAC_TABLE 8            /* Dirac plans without a field, ndim >= 2: 0 = cos(E tau), sin(E tau)/E of every k point
                                             evaluated in the kinetic pass, 1 = read from a table (16 bytes per k point) */
+#define SSO_OPT_TILE_ORDER 9              /* order in which the passes walk their tiles: 0 = auto; otherwise value - 1 is a mask of
+                                            the passes that go from the highest address down (bit 0 contiguous-axis passes,
+                                            1 middle-axis forward, 2 middle-axis inverse, 3 kinetic); results do not depend on it */
 #define SSO_OPT_THREADS_PER_CTA 6        /* ring pipeline CTA size: 512 (128 regs/thread) or 384 (168); 0 = auto */
 
 #define SSO_MIN_AXIS 16   /* smallest supported axis length                       */
@@ -162,6 +165,40 @@ int sso_step_host(sso_plan *plan, void *psi_host, int64_t nsteps);
  * accumulated in double also for SSO_C64, in a fixed order (deterministic).  Synchronises `stream`.
  */
 int sso_norm(sso_plan *plan, const void *psi, double *out_host, void *stream);
+
+/*
+ * Observables (section V.2).  psi, psi_a, psi_b are DEVICE pointers laid out as for sso_step, in
+ * position space (i.e. between sso_step calls); results go to HOST memory; every sum is accumulated in double, also
+ * for SSO_C64, in a fixed order (deterministic); integrals are sums over the lattice times prod(dx).  All of these
+ * synchronise `stream` except sso_filter_accumulate.
+ *
+ * sso_overlap: out_host[0..1] = (re, im) of <a|b> = sum_c sum_r conj(a_c(r)) b_c(r) prod(dx) -- the autocorrelation
+ *   function chi(t) of PAPER.md:359 eq. 40 for a = Psi(., 0), b = Psi(., t).
+ * sso_expect_position: out_host[a] = sum r_a |psi|^2 prod(dx), a < ndim, on the grid r_j = (j - n/2) dx (reading G14).
+ * sso_expect_momentum: out_host[a] = sum_k k_a |psi~(k)|^2 prod(dx) / N, the canonical momentum (hbar = 1), psi~ the
+ *   unnormalised forward transform of PAPER.md:103 eq. 12 taken on a plan-owned copy (psi is not modified; the copy
+ *   is allocated on first use and costs as much device memory as psi).
+ */
+int sso_overlap(sso_plan *plan, const void *psi_a, const void *psi_b, double *out_host, void *stream);
+int sso_expect_position(sso_plan *plan, const void *psi, double *out_host, void *stream);
+int sso_expect_momentum(sso_plan *plan, const void *psi, double *out_host, void *stream);
+
+/*
+ * Windowed spectrum of an autocorrelation function (eq. 41):
+ *   out[e] = sum_{n < nt} chi(n dts) (1 - cos(2 pi n / nt)) exp(i n dts E[e]) dts,      T = nt dts,
+ * the integral of eq. 41 as the sum over the samples (reading G30).  chi_host: nt complex128 samples (re, im
+ * interleaved), E_host: nE energies, out_host: nE complex128 values; all HOST arrays, copied.  nt, nE > 0.
+ */
+int sso_spectrum(sso_plan *plan, const double *chi_host, int64_t nt, double dts, const double *E_host, int64_t nE,
+                 double *out_host, void *stream);
+
+/*
+ * One term of the eigenfunction filter (eq. 42):  acc(r) += psi(r) (1 - cos(2 pi t/T)) exp(i E t) dts
+ * for every component.  acc is a DEVICE array of ncomp * prod(sizes) complex128 numbers whatever the plan's
+ * precision (the caller zeroes it before the first term and owns it); psi as for sso_step.  Asynchronous on `stream`.
+ */
+int sso_filter_accumulate(sso_plan *plan, void *acc, const void *psi, double t, double T, double E, double dts,
+                          void *stream);
 
 /* Tuning knobs (SSO_OPT_*); invalid values give SSO_ERR_INVALID. */
 int sso_set_option(sso_plan *plan, int option, int64_t value);

@@ -21,14 +21,15 @@ OK, ERR_INVALID, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_STATE = 0, 1, 2, 3, 4
 C64, C128 = 0, 1
 FIELD_NONE, FIELD_E, FIELD_A = 0, 1, 2
 OPT_LINES_PER_TILE_CONTIG, OPT_LINES_PER_TILE_STRIDED, OPT_POTENTIAL_PHASE = 1, 2, 3
-OPT_GROUPS_PER_CTA, OPT_RING_BUFFERS, OPT_THREADS_PER_CTA, OPT_STRIDED_RING, OPT_DIRAC_TABLE = 4, 5, 6, 7, 8
+OPT_GROUPS_PER_CTA, OPT_RING_BUFFERS, OPT_THREADS_PER_CTA, OPT_STRIDED_RING, OPT_DIRAC_TABLE, OPT_TILE_ORDER = 4, 5, 6, 7, 8, 9
 
 # every symbol include/sso.h declares
 SYMBOLS = (
     "sso_plan_create", "sso_set_constants", "sso_set_potential", "sso_set_field", "sso_set_time_index",
     "sso_get_time_index", "sso_step", "sso_step_host", "sso_norm", "sso_set_option", "sso_launch_count",
     "sso_destroy", "sso_last_error", "sso_version", "sso_debug_layout", "sso_profile_step", "sso_pass_name",
-    "sso_set_vector_potential",
+    "sso_set_vector_potential", "sso_overlap", "sso_expect_position", "sso_expect_momentum", "sso_spectrum",
+    "sso_filter_accumulate",
 )
 PASS_KINDS = 9
 
@@ -68,6 +69,11 @@ def lib() -> ctypes.CDLL:
         L.sso_version.restype = ctypes.c_char_p
         L.sso_profile_step.argtypes = [vp, vp, i64, vp, ctypes.POINTER(i64), ctypes.POINTER(dbl)]
         L.sso_pass_name.argtypes = [ci]
+        L.sso_overlap.argtypes = [vp, vp, vp, ctypes.POINTER(dbl), vp]
+        L.sso_expect_position.argtypes = [vp, vp, ctypes.POINTER(dbl), vp]
+        L.sso_expect_momentum.argtypes = [vp, vp, ctypes.POINTER(dbl), vp]
+        L.sso_spectrum.argtypes = [vp, vp, i64, dbl, vp, i64, vp, vp]
+        L.sso_filter_accumulate.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp]
         L.sso_pass_name.restype = ctypes.c_char_p
         for name in SYMBOLS:
             if name not in ("sso_last_error", "sso_version", "sso_pass_name"):
@@ -197,6 +203,41 @@ class Plan:
         _check_buffer(psi, self._psi_bytes, self._esz, True, "psi")
         self._ck(lib().sso_norm(self._h, _ptr(psi), ctypes.byref(out), _stream(stream)))
         return out.value
+
+    # observables
+    def overlap(self, psi_a, psi_b, stream=None) -> complex:
+        """<a|b> = sum conj(a) b prod dx (chi(t) of eq. 40 for a = psi(0), b = psi(t))."""
+        _check_buffer(psi_a, self._psi_bytes, self._esz, True, "psi_a")
+        _check_buffer(psi_b, self._psi_bytes, self._esz, True, "psi_b")
+        out = (ctypes.c_double * 2)()
+        self._ck(lib().sso_overlap(self._h, _ptr(psi_a), _ptr(psi_b), out, _stream(stream)))
+        return complex(out[0], out[1])
+
+    def expect_position(self, psi, stream=None):
+        _check_buffer(psi, self._psi_bytes, self._esz, True, "psi")
+        out = (ctypes.c_double * 3)()
+        self._ck(lib().sso_expect_position(self._h, _ptr(psi), out, _stream(stream)))
+        return [out[a] for a in range(len(self.sizes))]
+
+    def expect_momentum(self, psi, stream=None):
+        _check_buffer(psi, self._psi_bytes, self._esz, True, "psi")
+        out = (ctypes.c_double * 3)()
+        self._ck(lib().sso_expect_momentum(self._h, _ptr(psi), out, _stream(stream)))
+        return [out[a] for a in range(len(self.sizes))]
+
+    def spectrum(self, chi, dts: float, E, out, stream=None) -> None:
+        """chi: complex128 host array [nt]; E: float64 host array [nE]; out: complex128 host array [nE], filled."""
+        nt, nE = chi.shape[0], E.shape[0]
+        _check_buffer(chi, nt * 16, 16, False, "chi")
+        _check_buffer(E, nE * 8, 8, False, "E")
+        _check_buffer(out, nE * 16, 16, False, "out")
+        self._ck(lib().sso_spectrum(self._h, _ptr(chi), int(nt), float(dts), _ptr(E), int(nE), _ptr(out), _stream(stream)))
+
+    def filter_accumulate(self, acc, psi, t: float, T: float, E: float, dts: float, stream=None) -> None:
+        """acc (complex128 CUDA tensor, shape of psi) += psi (1 - cos(2 pi t/T)) exp(i E t) dts (one term of eq. 42)."""
+        _check_buffer(acc, self._npts * self.ncomp * 16, 16, True, "acc")
+        _check_buffer(psi, self._psi_bytes, self._esz, True, "psi")
+        self._ck(lib().sso_filter_accumulate(self._h, _ptr(acc), _ptr(psi), float(t), float(T), float(E), float(dts), _stream(stream)))
 
     def profile_step(self, psi, nsteps: int, stream=None):
         """sso_profile_step: [(pass name, launches, mean microseconds)] for the pass kinds that ran."""

@@ -79,16 +79,14 @@ __global__ void build_kphase_kernel(const double *__restrict__ kv, void *__restr
     reinterpret_cast<C *>(out)[i] = h;
 }
 
-// Dirac kinetic pass tables.  cp0[s] = c (k_0[s] - sh0) for every slot s of axis 0; and, when `out` is given, the
-// kinetic scalars of every k point in the order the pass meets them ([slot along axis 0][the other axes in storage
-// order]):  out = scale * (cos(E tau), sin(E tau)/E),  E = sqrt(c^2 |k - sh|^2 + m^2 c^4), sh = q Abar_n
-// (eq. 32; closed form of eq. 33, see sso_sring.cuh; reading G16 for the shift)
-__global__ void build_ktab_kernel(double2 *__restrict__ out, double *__restrict__ cp0, const double *__restrict__ kv0,
-                                  const double *__restrict__ kv1, const double *__restrict__ kv2, int n0, long long total, long long inner,
-                                  int rest1, double sh0, double sh1, double sh2, double mass, double clight, double dt, double scale) {
+// Dirac kinetic scalars of every k point (SSO_OPT_DIRAC_TABLE = 1) in the order the pass meets them ([slot along
+// axis 0][the other axes in storage order]):  out = scale * (cos(E tau), sin(E tau)/E),
+// E = sqrt(c^2 |k - sh|^2 + m^2 c^4), sh = q Abar_n   (eq. 32; closed form of eq. 33, see
+// sso_sring.cuh; reading G16 for the shift)
+__global__ void build_ktab_kernel(double2 *__restrict__ out, const double *__restrict__ kv0, const double *__restrict__ kv1,
+                                  const double *__restrict__ kv2, long long total, long long inner, int rest1, double sh0, double sh1,
+                                  double sh2, double mass, double clight, double dt, double scale) {
     const long long tid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (tid < n0) cp0[tid] = clight * (kv0[tid] - sh0);
-    if (!out) return;
     const double mc2 = mass * clight * clight;
     for (long long i = tid; i < total; i += (long long)gridDim.x * blockDim.x) {
         const long long s = i / inner, line = i % inner;
@@ -212,6 +210,126 @@ __global__ void norm_final_kernel(const double *__restrict__ partial, int n, dou
     if (threadIdx.x == 0) *out = acc * vol;
 }
 
+
+// ---- observables (section V.2) ---------------------------------------------------------------
+// block-level sum of NV doubles per thread: warp-shuffle tree, then one warp over the per-warp sums; fixed order.
+// On return thread 0 holds the sums in acc.
+template <int NV> __device__ __forceinline__ void block_sum(double (&acc)[NV]) {
+    __shared__ double wsum[NV][32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+        for (int o = 16; o > 0; o >>= 1) acc[v] += __shfl_down_sync(0xffffffffu, acc[v], o);
+        if (lane == 0) wsum[v][w] = acc[v];
+    }
+    __syncthreads();
+    if (w == 0) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            double t = lane < (int)(blockDim.x >> 5) ? wsum[v][lane] : 0.0;
+            for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+            acc[v] = t;
+        }
+    }
+}
+template <int NV> __device__ __forceinline__ void block_sum_store(double (&acc)[NV], double *__restrict__ partial) {
+    block_sum<NV>(acc);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) partial[v * gridDim.x + blockIdx.x] = acc[v];
+    }
+}
+// out[v] = scale * sum_b partial[v][b], one warp per value
+__global__ void reduce_final_kernel(const double *__restrict__ partial, int nblocks, int nv, double scale, double *__restrict__ out) {
+    const int v = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (v >= nv) return;
+    double acc = 0.0;
+    for (int i = lane; i < nblocks; i += 32) acc += partial[v * nblocks + i];
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+    if (lane == 0) out[v] = acc * scale;
+}
+
+// <a|b> = sum conj(a) b: the autocorrelation function chi(t) of PAPER.md:359 eq. 40 for a = Psi(0), b = Psi(t)
+template <typename T>
+__global__ void overlap_partial_kernel(const void *__restrict__ a_, const void *__restrict__ b_, long long count, double *__restrict__ partial) {
+    using C = typename Cx2<T>::type;
+    const C *a = reinterpret_cast<const C *>(a_), *b = reinterpret_cast<const C *>(b_);
+    double acc[2] = {0.0, 0.0};
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < count; i += (long long)gridDim.x * blockDim.x) {
+        const C u = a[i], v = b[i];
+        acc[0] += (double)u.x * (double)v.x + (double)u.y * (double)v.y;
+        acc[1] += (double)u.x * (double)v.y - (double)u.y * (double)v.x;
+    }
+    block_sum_store<2>(acc, partial);
+}
+
+// sum over the lattice of w_a(i_a) |psi(i)|^2 for every axis a, the density summed over the components.
+// Position expectation: tab = NULL, w_a(i) = (i - n_a/2) dx_a (grid of reading G14); momentum expectation: psi holds
+// the transform in network order on every axis and w_a(i) = tab[a][i], the momentum at network position i.
+struct AxisWeights {
+    const double *tab[3];
+    int n[3];
+    double dx[3];
+    int ndim, ncomp;
+    long long npts;
+};
+template <typename T> __global__ void weighted_density_partial_kernel(const void *__restrict__ psi_, const AxisWeights aw, double *__restrict__ partial) {
+    using C = typename Cx2<T>::type;
+    const C *psi = reinterpret_cast<const C *>(psi_);
+    double acc[3] = {0.0, 0.0, 0.0};
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < aw.npts; j += (long long)gridDim.x * blockDim.x) {
+        double d = 0.0;
+        for (int c = 0; c < aw.ncomp; ++c) {
+            const C v = psi[(long long)c * aw.npts + j];
+            d += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
+        }
+        long long rem = j;
+        for (int a = aw.ndim - 1; a >= 0; --a) {
+            const int ia = (int)(rem % aw.n[a]);
+            rem /= aw.n[a];
+            const double wgt = aw.tab[a] ? aw.tab[a][ia] : ((double)ia - (double)(aw.n[a] / 2)) * aw.dx[a];
+            acc[a] += wgt * d;
+        }
+    }
+    block_sum_store<3>(acc, partial);
+}
+
+// chi~(E) = sum_n chi(t_n) (1 - cos(2 pi t_n/T)) exp(i t_n E) dts, t_n = n dts, T = nt dts (eq. 41; the
+// integral as the sum over the samples, reading G30).  One block per energy.
+__global__ void spectrum_kernel(const double2 *__restrict__ chi, long long nt, double dts, const double *__restrict__ E, double2 *__restrict__ out) {
+    const double e = E[blockIdx.x];
+    double acc[2] = {0.0, 0.0};
+    for (long long n = threadIdx.x; n < nt; n += blockDim.x) {
+        const double wdw = 1.0 - cospi(2.0 * (double)n / (double)nt);  // t_n / T = n / nt
+        double sn, cs;
+        sincos((double)n * dts * e, &sn, &cs);
+        const double2 c = chi[n];
+        acc[0] += wdw * (c.x * cs - c.y * sn);
+        acc[1] += wdw * (c.x * sn + c.y * cs);
+    }
+    block_sum<2>(acc);
+    if (threadIdx.x == 0) out[blockIdx.x] = make_double2(acc[0] * dts, acc[1] * dts);
+}
+
+// acc += psi (1 - cos(2 pi t/T)) exp(i E t) dts, one term of PAPER.md:367 eq. 42; acc is complex128 whatever psi is
+template <typename T>
+__global__ void filter_accumulate_kernel(double2 *__restrict__ acc, const void *__restrict__ psi_, long long count, double t, double Ttot, double E, double dts) {
+    using C = typename Cx2<T>::type;
+    const C *psi = reinterpret_cast<const C *>(psi_);
+    double wi, wr;
+    sincos(E * t, &wi, &wr);
+    const double wdw = (1.0 - cospi(2.0 * t / Ttot)) * dts;
+    wr *= wdw;
+    wi *= wdw;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < count; i += (long long)gridDim.x * blockDim.x) {
+        const C v = psi[i];
+        double2 a = acc[i];
+        a.x += wr * (double)v.x - wi * (double)v.y;
+        a.y += wr * (double)v.y + wi * (double)v.x;
+        acc[i] = a;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
@@ -311,6 +429,7 @@ struct Axis {
     int *d_slot_nat = nullptr;     // device int[n]
     double *d_kv = nullptr;        // device double[n]: k in the layout this axis uses in the kinetic pass
     void *d_kph = nullptr;         // device complex[n]: Schroedinger phase table in the same layout
+    double *d_kpos = nullptr;      // device double[n]: k at network position p (sso_expect_momentum)
 };
 
 }  // namespace sso
@@ -341,9 +460,9 @@ struct sso_plan {
     bool kph_valid = false;
     double *d_apos = nullptr; // step-averaged position-dependent A(r), [ndim][npts], or NULL (sso_set_vector_potential)
     void *d_ktab = nullptr;   // Dirac kinetic scalars per k point (SSO_OPT_DIRAC_TABLE = 1), else NULL
-    double *d_kcp0 = nullptr; // Dirac: c (k_0 - q Abar_0) per slot of axis 0
-    bool ktab_valid = false;  // both tables are current (plans without SSO_FIELD_A only; with it they change every step)
+    bool ktab_valid = false;  // the table is current (plans without SSO_FIELD_A only; with it it changes every step)
     int opt_dirac_table = 0;
+    int opt_tile_order = 0;   // SSO_OPT_TILE_ORDER
     int opt_tl_contig = 0, opt_tl_strided = 0, opt_groups = 0, opt_ring = 0, opt_maxt = 0, opt_sring = 0;
     int device = 0, num_sms = 0;  // the device the plan was created on, its SM count
     size_t smem_optin = 0;        // largest dynamic shared memory a CTA may opt in to on that device
@@ -353,7 +472,8 @@ struct sso_plan {
     };
     std::vector<ProfEvent> *prof = nullptr;  // non-NULL while sso_profile_step brackets every launch with events
     bool v_valid = true;          // false between a change of the potential representation and the next sso_set_potential
-    double *d_partial = nullptr, *d_norm = nullptr;
+    double *d_partial = nullptr, *d_norm = nullptr;  // reductions: [4][NORM_BLOCKS] partial sums, [4] results
+    void *d_scratch = nullptr;    // psi-sized work buffer of sso_expect_momentum (allocated on first use)
     unsigned *d_sched = nullptr;  // tile scheduler of the pass kernel (zero between launches)
     void *d_hostbuf = nullptr;
     std::string err;
@@ -546,14 +666,19 @@ int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double
         kinetic_layout(plan, a, kv);
         if (e == cudaSuccess) e = upload((void **)&A.d_kv, kv);
         if (e == cudaSuccess) e = cudaMalloc(&A.d_kph, (size_t)n * plan->esize());
+        {
+            std::vector<double> kpos(n);
+            for (int q = 0; q < n; ++q) kpos[q] = A.k_nat[A.pos_freq[q]];
+            if (e == cudaSuccess) e = upload((void **)&A.d_kpos, kpos);
+        }
         if (e != cudaSuccess) {
             int rc = cuda_fail(nullptr, e, "plan tables");
             sso_destroy(plan);
             return rc;
         }
     }
-    cudaError_t e = cudaMalloc((void **)&plan->d_partial, sizeof(double) * NORM_BLOCKS);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&plan->d_norm, sizeof(double));
+    cudaError_t e = cudaMalloc((void **)&plan->d_partial, sizeof(double) * 4 * NORM_BLOCKS);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&plan->d_norm, sizeof(double) * 4);
     if (e == cudaSuccess) e = cudaMalloc((void **)&plan->d_sched, 2 * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMemset(plan->d_sched, 0, 2 * sizeof(unsigned));
     if (e != cudaSuccess) {
@@ -581,18 +706,19 @@ int sso_destroy(sso_plan *plan) {
         cudaFree(A.d_slot_nat);
         cudaFree(A.d_kv);
         cudaFree(A.d_kph);
+        cudaFree(A.d_kpos);
     }
     cudaFree(plan->d_avg);
     cudaFree(plan->d_vtab);
     cudaFree(plan->d_vfull);
     cudaFree(plan->d_ktab);
-    cudaFree(plan->d_kcp0);
     cudaFree(plan->d_apos);
     for (int a = 0; a < 3; ++a) cudaFree(plan->d_erow[a]);
     cudaFree(plan->d_partial);
     cudaFree(plan->d_norm);
     cudaFree(plan->d_sched);
     cudaFree(plan->d_hostbuf);
+    cudaFree(plan->d_scratch);
     delete plan;
     return SSO_OK;
 }
@@ -782,6 +908,10 @@ int sso_set_option(sso_plan *plan, int option, int64_t value) {
             }
             plan->ktab_valid = false;
             return SSO_OK;
+        case SSO_OPT_TILE_ORDER:
+            if (value < 0 || value > 16) return fail(plan, SSO_ERR_INVALID, "tile order must be in [0, 16]");
+            plan->opt_tile_order = (int)value;
+            return SSO_OK;
         case SSO_OPT_POTENTIAL_PHASE:
             if (value != VREP_TABLE && value != VREP_ANGLE) return fail(plan, SSO_ERR_INVALID, "potential phase mode must be 0 or 1");
             if ((int)value != plan->vrep) {
@@ -835,6 +965,15 @@ Geometry geometry(const sso_plan *p, int axis) {
         g.rest1 = p->ax[others[1]].n;
     }
     return g;
+}
+
+// Which passes walk their tiles from the highest address down (bit 0: contiguous-axis passes, 1: middle-axis
+// forward, 2: middle-axis inverse, 3: kinetic).  A pass that starts where the previous one ended finds that part of
+// psi still in L2 (and its dirty lines are overwritten there instead of going to HBM twice): with the contiguous-axis
+// passes descending and the middle-axis passes ascending, every plane-ordered hand-over of a 3D step meets that way.
+int tile_order_mask(const sso_plan *p) {
+    if (p->opt_tile_order > 0) return p->opt_tile_order - 1;
+    return p->ndim == 3 ? 1 : 0;
 }
 
 // lines per component per CTA
@@ -1028,6 +1167,7 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     a.rest1 = g.rest1;
     a.vtab = mode == MODE_MID ? plan->d_vfull : plan->d_vtab;
     a.vrep = plan->vrep;
+    a.rev = tile_order_mask(plan) & 1;
     if (plan->field_kind == SSO_FIELD_E) {
         if (plan->e_axis_on[last]) a.eline = (const char *)plan->d_erow[last] + (size_t)row * A.n * esz;
         if (g.oaxA >= 0 && plan->e_axis_on[g.oaxA]) a.eoA = (const char *)plan->d_erow[g.oaxA] + (size_t)row * plan->ax[g.oaxA].n * esz;
@@ -1172,6 +1312,7 @@ int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long 
     if (ntiles > 0x7fffffffLL) return fail(plan, SSO_ERR_UNSUPPORTED, "too many tiles");
     a.ntiles = (int)ntiles;
     a.ndim = plan->ndim;
+    a.rev = (tile_order_mask(plan) >> (smode == SMODE_DIF ? 1 : (smode == SMODE_DIT ? 2 : 3))) & 1;
     a.mass = plan->mass;
     a.clight = plan->clight;
     a.dt = plan->dt;
@@ -1186,7 +1327,16 @@ int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long 
         a.kv2 = g.oaxB >= 0 ? plan->ax[g.oaxB].d_kv : nullptr;
         if (plan->field_kind == SSO_FIELD_A)
             for (int ax = 0; ax < plan->ndim; ++ax) a.sh[ax] = plan->charge * plan->h_avg[(size_t)n * plan->ndim + ax];
-        a.kcp0 = plan->d_kcp0;
+        {   // largest |E tau| of the plan: below 2^30 the kernel's own quadrant reduction is exact enough
+            double p2max = 0.0;
+            for (int ax = 0; ax < plan->ndim; ++ax) {
+                const double km = 3.14159265358979323846 / plan->ax[ax].dx + fabs(a.sh[ax]);
+                p2max += km * km;
+            }
+            const double mc2 = plan->mass * plan->clight * plan->clight;
+            const double emax = sqrt(plan->clight * plan->clight * p2max + mc2 * mc2);
+            a.fast_trig = emax * fabs(plan->dt) < 1073741824.0 ? 1 : 0;
+        }
         a.ktab = plan->d_ktab;
         if (!plan->opt_dirac_table) smode = smode == SMODE_KD2 ? SMODE_KD2F : SMODE_KD4F;
     }
@@ -1274,17 +1424,13 @@ int build_kphase(sso_plan *plan, long long n, cudaStream_t st) {
     return SSO_OK;
 }
 
-// tables of the Dirac kinetic pass (build_ktab_kernel): built once for a plan without SSO_FIELD_A, every step with it
-bool dirac_tables_per_step(const sso_plan *p) { return p->ncomp > 1 && p->ndim >= 2 && p->field_kind == SSO_FIELD_A; }
+// table of the Dirac kinetic scalars (SSO_OPT_DIRAC_TABLE = 1): built once for a plan without SSO_FIELD_A, every step with it
+bool dirac_table_per_step(const sso_plan *p) { return p->opt_dirac_table && p->ncomp > 1 && p->ndim >= 2 && p->field_kind == SSO_FIELD_A; }
 int build_ktab(sso_plan *plan, long long n, cudaStream_t st) {
-    if (plan->ncomp == 1 || plan->ndim < 2) return SSO_OK;
+    if (plan->ncomp == 1 || plan->ndim < 2 || !plan->opt_dirac_table) return SSO_OK;
     const bool shifted = plan->field_kind == SSO_FIELD_A;
     if (plan->ktab_valid && !shifted) return SSO_OK;
-    if (!plan->d_kcp0) {
-        cudaError_t e = cudaMalloc((void **)&plan->d_kcp0, sizeof(double) * (size_t)plan->ax[0].n);
-        if (e != cudaSuccess) return fail(plan, SSO_ERR_ALLOC, std::string("Dirac momentum table: ") + cudaGetErrorString(e));
-    }
-    if (plan->opt_dirac_table && !plan->d_ktab) {
+    if (!plan->d_ktab) {
         cudaError_t e = cudaMalloc(&plan->d_ktab, sizeof(double2) * (size_t)plan->npts);
         if (e != cudaSuccess) return fail(plan, SSO_ERR_ALLOC, std::string("Dirac kinetic table: ") + cudaGetErrorString(e));
     }
@@ -1293,12 +1439,10 @@ int build_ktab(sso_plan *plan, long long n, cudaStream_t st) {
         for (int ax = 0; ax < plan->ndim; ++ax) sh[ax] = plan->charge * plan->h_avg[(size_t)n * plan->ndim + ax];
     PassTimer timer(plan, SSO_PASS_TABLES, st);
     const Geometry g = geometry(plan, 0);
-    const bool table = plan->opt_dirac_table != 0;
-    const int blocks = table ? plan->num_sms * 8 : (plan->ax[0].n + 255) / 256;
-    build_ktab_kernel<<<blocks, 256, 0, st>>>(table ? reinterpret_cast<double2 *>(plan->d_ktab) : nullptr, plan->d_kcp0, plan->ax[0].d_kv,
-                                             g.oaxA >= 0 ? plan->ax[g.oaxA].d_kv : nullptr, g.oaxB >= 0 ? plan->ax[g.oaxB].d_kv : nullptr,
-                                             plan->ax[0].n, plan->npts, g.inner, g.rest1, sh[0], sh[1], sh[2], plan->mass, plan->clight, plan->dt,
-                                             1.0 / (double)plan->npts);
+    build_ktab_kernel<<<plan->num_sms * 8, 256, 0, st>>>(reinterpret_cast<double2 *>(plan->d_ktab), plan->ax[0].d_kv,
+                                                        g.oaxA >= 0 ? plan->ax[g.oaxA].d_kv : nullptr, g.oaxB >= 0 ? plan->ax[g.oaxB].d_kv : nullptr,
+                                                        plan->npts, g.inner, g.rest1, sh[0], sh[1], sh[2], plan->mass, plan->clight, plan->dt,
+                                                        1.0 / (double)plan->npts);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(plan, e, "Dirac kinetic table kernel");
     plan->ktab_valid = !shifted;
@@ -1319,7 +1463,7 @@ long long launches_for(const sso_plan *p, long long nsteps) {
     }
     const long long chunk = p->d_apos ? 1 : erow_chunk(p);
     const long long nchunks = (nsteps + chunk - 1) / chunk;
-    if (p->ncomp > 1 && sring_shape(p, 0, p->ncomp, false).ok) cnt += dirac_tables_per_step(p) ? nsteps : (p->ktab_valid ? 0 : 1);  // Dirac kinetic tables
+    if (p->ncomp > 1 && p->opt_dirac_table && sring_shape(p, 0, p->ncomp, false).ok) cnt += dirac_table_per_step(p) ? nsteps : (p->ktab_valid ? 0 : 1);  // Dirac kinetic table
     bool eph = false;
     for (int a = 0; a < p->ndim; ++a) eph = eph || (p->field_kind == SSO_FIELD_E && p->e_axis_on[a]);
     cnt += nchunks * (eph ? 2 : 1);              // opening pass (+ field phase rows)
@@ -1510,6 +1654,112 @@ int sso_norm(sso_plan *plan, const void *psi, double *out_host, void *stream) {
     CK(cudaGetLastError());
     CK(cudaMemcpyAsync(out_host, plan->d_norm, sizeof(double), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    return SSO_OK;
+}
+
+// ---- observables -------------------------------------------------------------------------------
+
+int sso_overlap(sso_plan *plan, const void *psi_a, const void *psi_b, double *out_host, void *stream) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (!psi_a || !psi_b || !out_host) return fail(plan, SSO_ERR_INVALID, "psi_a, psi_b or out_host is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long count = plan->npts * plan->ncomp;
+    double vol = 1.0;
+    for (int a = 0; a < plan->ndim; ++a) vol *= plan->ax[a].dx;
+    if (plan->precision == SSO_C128) overlap_partial_kernel<double><<<NORM_BLOCKS, 256, 0, st>>>(psi_a, psi_b, count, plan->d_partial);
+    else overlap_partial_kernel<float><<<NORM_BLOCKS, 256, 0, st>>>(psi_a, psi_b, count, plan->d_partial);
+    reduce_final_kernel<<<1, 64, 0, st>>>(plan->d_partial, NORM_BLOCKS, 2, vol, plan->d_norm);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(out_host, plan->d_norm, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return SSO_OK;
+}
+
+static int weighted_density(sso_plan *plan, const void *psi, bool momentum, double scale, double *out_host, cudaStream_t st) {
+    AxisWeights aw{};
+    for (int a = 0; a < 3; ++a) {
+        aw.tab[a] = (momentum && a < plan->ndim) ? plan->ax[a].d_kpos : nullptr;
+        aw.n[a] = a < plan->ndim ? plan->ax[a].n : 1;
+        aw.dx[a] = a < plan->ndim ? plan->ax[a].dx : 1.0;
+    }
+    aw.ndim = plan->ndim;
+    aw.ncomp = plan->ncomp;
+    aw.npts = plan->npts;
+    if (plan->precision == SSO_C128) weighted_density_partial_kernel<double><<<NORM_BLOCKS, 256, 0, st>>>(psi, aw, plan->d_partial);
+    else weighted_density_partial_kernel<float><<<NORM_BLOCKS, 256, 0, st>>>(psi, aw, plan->d_partial);
+    reduce_final_kernel<<<1, 96, 0, st>>>(plan->d_partial, NORM_BLOCKS, 3, scale, plan->d_norm);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(out_host, plan->d_norm, (size_t)plan->ndim * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return SSO_OK;
+}
+
+int sso_expect_position(sso_plan *plan, const void *psi, double *out_host, void *stream) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (!psi || !out_host) return fail(plan, SSO_ERR_INVALID, "psi or out_host is NULL");
+    double vol = 1.0;
+    for (int a = 0; a < plan->ndim; ++a) vol *= plan->ax[a].dx;
+    return weighted_density(plan, psi, false, vol, out_host, (cudaStream_t)stream);
+}
+
+int sso_expect_momentum(sso_plan *plan, const void *psi, double *out_host, void *stream) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (!psi || !out_host) return fail(plan, SSO_ERR_INVALID, "psi or out_host is NULL");
+    if (((uintptr_t)psi & 15u) != 0) return fail(plan, SSO_ERR_INVALID, "psi must be 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)plan->npts * plan->ncomp * plan->esize();
+    if (!plan->d_scratch) {
+        cudaError_t e = cudaMalloc(&plan->d_scratch, bytes);
+        if (e != cudaSuccess) return fail(plan, SSO_ERR_ALLOC, std::string("work buffer: ") + cudaGetErrorString(e));
+    }
+    CK(cudaMemcpyAsync(plan->d_scratch, psi, bytes, cudaMemcpyDeviceToDevice, st));
+    // forward transform of the copy along every axis, left in network order (the momentum table is stored that way)
+    for (int a = 0; a < plan->ndim; ++a) {
+        const bool contiguous = a == plan->ndim - 1;
+        PassSpec ps{a, contiguous ? PW_KS : PW_NONE, -1, 1, 0, 0, 0, 0, 0, 1, 0};
+        const int rc = launch(plan, plan->d_scratch, ps, st);
+        if (rc != SSO_OK) return rc;
+    }
+    double vol = 1.0;
+    for (int a = 0; a < plan->ndim; ++a) vol *= plan->ax[a].dx;
+    return weighted_density(plan, plan->d_scratch, true, vol / (double)plan->npts, out_host, st);
+}
+
+int sso_spectrum(sso_plan *plan, const double *chi_host, int64_t nt, double dts, const double *E_host, int64_t nE, double *out_host, void *stream) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (!chi_host || !E_host || !out_host) return fail(plan, SSO_ERR_INVALID, "chi_host, E_host or out_host is NULL");
+    if (nt <= 0 || nE <= 0 || nE > 0x7fffffffLL || !isfinite(dts)) return fail(plan, SSO_ERR_INVALID, "nt and nE must be positive, dts finite");
+    cudaStream_t st = (cudaStream_t)stream;
+    double2 *d_chi = nullptr, *d_out = nullptr;
+    double *d_E = nullptr;
+    cudaError_t e = cudaMalloc((void **)&d_chi, sizeof(double2) * (size_t)nt);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&d_E, sizeof(double) * (size_t)nE);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&d_out, sizeof(double2) * (size_t)nE);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_chi, chi_host, sizeof(double2) * (size_t)nt, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_E, E_host, sizeof(double) * (size_t)nE, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        spectrum_kernel<<<(unsigned)nE, 256, 0, st>>>(d_chi, nt, dts, d_E, d_out);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out_host, d_out, sizeof(double2) * (size_t)nE, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d_chi);
+    cudaFree(d_E);
+    cudaFree(d_out);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "sso_spectrum");
+    return SSO_OK;
+}
+
+int sso_filter_accumulate(sso_plan *plan, void *acc, const void *psi, double t, double T, double E, double dts, void *stream) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (!acc || !psi) return fail(plan, SSO_ERR_INVALID, "acc or psi is NULL");
+    if (!(T > 0.0) || !isfinite(t) || !isfinite(T) || !isfinite(E) || !isfinite(dts)) return fail(plan, SSO_ERR_INVALID, "T must be positive, all arguments finite");
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long count = plan->npts * plan->ncomp;
+    const int blocks = plan->num_sms * 8;
+    if (plan->precision == SSO_C128) filter_accumulate_kernel<double><<<blocks, 256, 0, st>>>(reinterpret_cast<double2 *>(acc), psi, count, t, T, E, dts);
+    else filter_accumulate_kernel<float><<<blocks, 256, 0, st>>>(reinterpret_cast<double2 *>(acc), psi, count, t, T, E, dts);
+    CK(cudaGetLastError());
     return SSO_OK;
 }
 

@@ -88,6 +88,7 @@ struct RingArgs {
     int vrep;                 // VREP_TABLE (complex phases) or VREP_ANGLE (real angles, sincos in the kernel)
     const void *eline;        // complex[N] field phase along the line for this pass (same order as vtab) or NULL
     const void *eoA, *eoB;    // complex field phase rows of the other axes, indexed by ia / ib, or NULL
+    int rev;                  // tiles in descending address order
 };
 
 using RingLaunchFn = cudaError_t (*)(const RingArgs &, unsigned threads, size_t smem, unsigned grid, cudaStream_t st);
@@ -112,9 +113,10 @@ struct SRingArgs {
     const double *kv0, *kv1, *kv2;   // Dirac k grids (PassArgs)
     double sh[3];                    // q Abar_n per axis (SSO_FIELD_A), else 0
     const void *ktab;                // Dirac table modes: double2 (cos(E tau), sin(E tau)/E) / Ntot per k point, [slot of axis 0][inner]
-    const double *kcp0;              // Dirac: c (k_0 - q Abar_0) per slot of axis 0
     double mass, clight, dt, scale;
     int ndim;
+    int rev;                         // tiles in descending order
+    int fast_trig;                   // Dirac: |E tau| < 2^30 for every k point, the kernel may use its own quadrant reduction
 };
 // bytes of the line table a strided pass keeps in shared memory (multiple of 128): the Schroedinger kinetic phases
 // of the line axis (complex[N]) or the Dirac momenta c (k_0 - q Abar_0) (double[N])

@@ -171,8 +171,14 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
         *table_line = lb * TL;
         return (comp * a.lines_per_comp + lb * TL) * (long long)N;
     };
+    // CTA-local tile k -> global tile.  rev: highest addresses first, so that this pass starts on what the previous
+    // pass of the stream (which ended there) left in L2 and ends on the lowest addresses, where the next one starts
+    auto tile_of = [&](int k) -> long long {
+        const long long tl = (long long)blockIdx.x + (long long)k * gridDim.x;
+        return a.rev ? (long long)a.ntiles - 1 - tl : tl;
+    };
     auto issue = [&](int k, int b) {
-        const long long tile = (long long)blockIdx.x + (long long)k * gridDim.x;
+        const long long tile = tile_of(k);
         long long l0;
         const long long e0 = tile_elem(tile, &l0);
         mbar_expect_tx(&full[b], tile_bytes);
@@ -219,7 +225,7 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
         C *buf = bufs + (size_t)b * a.bufstride;
         C *dense = buf + t * N + u;          // bulk-copy layout: [TL][N]
         C *sl = buf + t * a.pitch;           // exchange layout: padded lines
-        const long long tile = (long long)blockIdx.x + (long long)k * gridDim.x;
+        const long long tile = tile_of(k);
         long long l0_;
         const long long e0_ = tile_elem(tile, &l0_);
         const int lic = (int)l0_ + t;  // line within the component = table line

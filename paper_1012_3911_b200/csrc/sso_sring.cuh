@@ -31,19 +31,30 @@ __device__ __forceinline__ void tma_load_3d(void *smem_dst, const CUtensorMap *m
 template <int CC> struct DiracScalars {
     double cs[16 / CC], sE[16 / CC];  // cos(E tau) / Ntot and sin(E tau) / (E Ntot) of those k points
 };
-// evaluated while x is parked in shared memory (inside the last exchange of the forward transform), so that sqrt and
-// sincos run with the registers of x free.  r12 = c^2 (pi_1^2 + pi_2^2) + m^2 c^4 is the same for the whole line.
+// evaluated while x is parked in shared memory (inside the last exchange of the forward transform), so that the
+// square root and the trigonometric pair run with the registers of x free.  r12 = c^2 (pi_1^2 + pi_2^2) + m^2 c^4 is
+// the same for the whole line.  E^2 >= m^2 c^4 > 0, so 1/E comes from one rsqrt (E = E^2 rsqrt(E^2), a few ulp) and no
+// division; FAST: |E tau| < 2^30 for every k point of the plan (checked on the host), so the quadrant reduction of
+// expi_small replaces the library sincos.  Together about 40 FP64 instructions per k point against about 85.
 template <int CC, int U>
-__device__ __forceinline__ void dirac_scalars(DiracScalars<CC> &k, int u, int c, const double *cp0, double r12, double dt, double scale) {
+__device__ __forceinline__ void dirac_scalars(DiracScalars<CC> &k, int u, int c, const double *cp0, double r12, double dt, double scale, bool fast) {
     constexpr int PP = 16 / CC;
 #pragma unroll
     for (int i = 0; i < PP; ++i) {
         const double w0 = cp0[(c * PP + i) * U + u];
-        const double E = sqrt(w0 * w0 + r12);
+        const double E2 = fma(w0, w0, r12);
+        const double rE = rsqrt(E2);
+        const double E = E2 * rE;
         double sn, cs;
-        sincos(E * dt, &sn, &cs);
+        if (fast) {
+            const double2 e = expi_small<double>(E * dt);
+            cs = e.x;
+            sn = e.y;
+        } else {
+            sincos(E * dt, &sn, &cs);
+        }
         k.cs[i] = cs * scale;
-        k.sE[i] = (E > 0.0 ? sn / E : dt) * scale;
+        k.sE[i] = sn * rE * scale;
     }
 }
 
@@ -151,7 +162,10 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
     const int nloc = a.ntiles > (int)blockIdx.x ? (a.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const int nbox = N / a.box_rows;
 
-    auto tile_of = [&](int k) { return (int)blockIdx.x + k * (int)gridDim.x; };
+    auto tile_of = [&](int k) {
+        const int tl = (int)blockIdx.x + k * (int)gridDim.x;
+        return a.rev ? a.ntiles - 1 - tl : tl;  // rev: see sso_ring.cuh
+    };
     auto issue = [&](int k, int b) {
         const int tile = tile_of(k);
         const int o = tile / a.tiles_per_outer, i0 = (tile % a.tiles_per_outer) * TL;
@@ -180,10 +194,15 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
         for (int j = 0; j < ring.owned(grp); ++j) refill(grp + G * j, grp + G * j);
     if constexpr (LTB > 0) {
         // (the line table may have been rebuilt for this step by the kernel before this one, hence after the wait)
-        const double *__restrict__ src = reinterpret_cast<const double *>(SMODE == SMODE_KS ? a.kph0 : (const void *)a.kcp0);
         double *dst = reinterpret_cast<double *>(ltab);
-        constexpr int ND = (SMODE == SMODE_KS ? N * (int)sizeof(C) : N * 8) / 8;
-        for (int i = threadIdx.x; i < ND; i += blockDim.x) dst[i] = src[i];
+        if constexpr (SMODE == SMODE_KS) {
+            const double *__restrict__ src = reinterpret_cast<const double *>(a.kph0);
+            constexpr int ND = N * (int)sizeof(C) / 8;
+            for (int i = threadIdx.x; i < ND; i += blockDim.x) dst[i] = src[i];
+        } else {
+            // Dirac: c pi_0 = c (k_0 - q Abar_0) per slot of the line axis (reading G16)
+            for (int i = threadIdx.x; i < N; i += blockDim.x) dst[i] = a.clight * (a.kv0[i] - a.sh[0]);
+        }
         __syncthreads();
     }
 
@@ -218,18 +237,11 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
                 w2 = a.clight * (a.kv2[line % a.rest1] - a.sh[2]);
             }
         }
-        if constexpr (SMODE == SMODE_DIT) {
-        } else if constexpr (CC > 1 && !KTABLE) {
-            const double r12 = w1 * w1 + w2 * w2 + mc2 * mc2;
-            DifChain<T, N, 0, -1>::run(x, u, stw, sl, gb, [&]() { dirac_scalars<CC, U>(dks, u, c, reinterpret_cast<const double *>(ltab), r12, a.dt, a.scale); });
-        } else {
-            DifChain<T, N, 0, -1>::run(x, u, stw, sl, gb);
-        }
-
+        // per-line factor of the Schroedinger kinetic phase (the other axes' tables), requested before the forward
+        // transform so that the loads are back when it ends
+        [[maybe_unused]] C s = mk<C>((T)1, (T)0);
+        [[maybe_unused]] bool has_s = false;
         if constexpr (SMODE == SMODE_KS) {
-            const C *k0 = reinterpret_cast<const C *>(ltab);
-            C s = mk<C>((T)1, (T)0);
-            bool has_s = false;
             if (a.kph1) {
                 s = reinterpret_cast<const C *>(a.kph1)[line / a.rest1];
                 has_s = true;
@@ -239,6 +251,17 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
                 s = has_s ? cmul(s, s2) : s2;
                 has_s = true;
             }
+        }
+        if constexpr (SMODE == SMODE_DIT) {
+        } else if constexpr (CC > 1 && !KTABLE) {
+            const double r12 = w1 * w1 + w2 * w2 + mc2 * mc2;
+            DifChain<T, N, 0, -1>::run(x, u, stw, sl, gb, [&]() { dirac_scalars<CC, U>(dks, u, c, reinterpret_cast<const double *>(ltab), r12, a.dt, a.scale, a.fast_trig != 0); });
+        } else {
+            DifChain<T, N, 0, -1>::run(x, u, stw, sl, gb);
+        }
+
+        if constexpr (SMODE == SMODE_KS) {
+            const C *k0 = reinterpret_cast<const C *>(ltab);
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
                 C f = k0[q * U + u];
@@ -260,12 +283,16 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
             const long long o = tile / a.tiles_per_outer;
             const long long i0 = (long long)(tile % a.tiles_per_outer) * TL;
             C *gout = reinterpret_cast<C *>(a.psi) + (CC > 1 ? (long long)c * a.comp_stride : o * (long long)N * a.inner) + i0 + t;
+            // one 64-bit multiply per thread, then pointer increments
             if constexpr (SMODE == SMODE_DIF) {
+                C *pq = gout + (long long)(u * 16) * a.inner;
 #pragma unroll
-                for (int q = 0; q < 16; ++q) st_stream(gout + (long long)(u * 16 + q) * a.inner, x[q]);
+                for (int q = 0; q < 16; ++q, pq += a.inner) st_stream(pq, x[q]);
             } else {
+                C *pq = gout + (long long)u * a.inner;
+                const long long rs = (long long)U * a.inner;
 #pragma unroll
-                for (int q = 0; q < 16; ++q) st_stream(gout + (long long)(u + q * U) * a.inner, x[q]);
+                for (int q = 0; q < 16; ++q, pq += rs) st_stream(pq, x[q]);
             }
         }
     }
