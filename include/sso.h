@@ -78,6 +78,7 @@ extern "C" {
 #define SSO_OPT_STRIDED_RING 7           /* strided-axis passes: 0 auto, 1 force the TMA ring, 2 direct kernel only */
 #define SSO_OPT_DIRAC_TABLE 8            /* Dirac plans without a field, ndim >= 2: 0 = cos(E tau), sin(E tau)/E of every k point
                                             evaluated in the kinetic pass, 1 = read from a table (16 bytes per k point) */
+#define SSO_OPT_LINES_PER_TILE_MIDDLE 10 /* adjacent lines per tile in the middle-axis passes of a 3D lattice (0 = auto)  */
 #define SSO_OPT_TILE_ORDER 9              /* order in which the passes walk their tiles: 0 = auto; otherwise value - 1 is a mask of
                                             the passes that go from the highest address down (bit 0 contiguous-axis passes,
                                             1 middle-axis forward, 2 middle-axis inverse, 3 kinetic); results do not depend on it */

@@ -463,6 +463,7 @@ struct sso_plan {
     bool ktab_valid = false;  // the table is current (plans without SSO_FIELD_A only; with it it changes every step)
     int opt_dirac_table = 0;
     int opt_tile_order = 0;   // SSO_OPT_TILE_ORDER
+    int opt_tl_middle = 0;    // SSO_OPT_LINES_PER_TILE_MIDDLE
     int opt_tl_contig = 0, opt_tl_strided = 0, opt_groups = 0, opt_ring = 0, opt_maxt = 0, opt_sring = 0;
     int device = 0, num_sms = 0;  // the device the plan was created on, its SM count
     size_t smem_optin = 0;        // largest dynamic shared memory a CTA may opt in to on that device
@@ -527,6 +528,11 @@ struct PassTimer {
 };
 
 static bool is_pow2(long long v) { return v > 0 && (v & (v - 1)) == 0; }
+static int ilog2ll(long long v) {
+    int l = 0;
+    while ((1LL << (l + 1)) <= v) ++l;
+    return l;
+}
 
 // which layout the kinetic tables of axis a use: axis 0 is the kinetic-sandwich axis (permuted slots),
 // the middle axis of a 3D lattice is stored in network order, the last axis of a >=2D lattice is natural
@@ -880,8 +886,9 @@ int sso_set_option(sso_plan *plan, int option, int64_t value) {
     switch (option) {
         case SSO_OPT_LINES_PER_TILE_CONTIG:
         case SSO_OPT_LINES_PER_TILE_STRIDED:
+        case SSO_OPT_LINES_PER_TILE_MIDDLE:
             if (value < 0 || value > 512 || (value > 0 && !is_pow2(value))) return fail(plan, SSO_ERR_INVALID, "lines per tile must be 0 or a power of two <= 512");
-            (option == SSO_OPT_LINES_PER_TILE_CONTIG ? plan->opt_tl_contig : plan->opt_tl_strided) = (int)value;
+            (option == SSO_OPT_LINES_PER_TILE_CONTIG ? plan->opt_tl_contig : (option == SSO_OPT_LINES_PER_TILE_STRIDED ? plan->opt_tl_strided : plan->opt_tl_middle)) = (int)value;
             return SSO_OK;
         case SSO_OPT_RING_BUFFERS:
             if (value < 0 || value > 16) return fail(plan, SSO_ERR_INVALID, "ring buffers must be in [0, 16]");
@@ -975,6 +982,9 @@ int tile_order_mask(const sso_plan *p) {
     if (p->opt_tile_order > 0) return p->opt_tile_order - 1;
     return p->ndim == 3 ? 1 : 0;
 }
+
+// shared-memory bytes of a pass's buffer pool state (sso_ring.cuh, TileRing::bytes): barriers, tiles, counters, mailboxes
+size_t ring_state_bytes(int nb, int g) { return (size_t)nb * 12 + 32 * 4 + 8 + (size_t)g * 4; }
 
 // lines per component per CTA
 int choose_tl(const sso_plan *p, const Geometry &g, int cc) {
@@ -1097,30 +1107,26 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
 }
 
 
-// groups per CTA and buffers per group of a ring pass: GT threads per group, room for bmax buffers,
-// tiles_per_cta tiles to share
-void choose_groups(const sso_plan *plan, int GT, int bmax, long long tiles_per_cta, int *G, int *NBG) {
-    int g = 1, nbg = bmax >= 2 ? 2 : 1;
+// groups per CTA and tile buffers of a contiguous-axis ring pass: GT threads per group, room for bmax buffers,
+// tiles_per_cta tiles to share.  As many groups as threads and buffers allow (measured: four groups beat three with
+// more buffers each); SSO_OPT_RING_BUFFERS adds spare buffers to the pool (sso_ring.cuh, TileRing).
+void choose_groups(const sso_plan *plan, int GT, int bmax, long long tiles_per_cta, int *G, int *NB) {
+    int g = 1;
     if (GT % 32 == 0) {
         const int cap = plan->opt_maxt ? plan->opt_maxt : 512;
         const int gthr = cap / GT > 15 ? 15 : cap / GT;
-        // as many groups as threads and buffers allow (measured: four single-buffered groups beat three
-        // double-buffered ones now that a buffer is refilled before its tile's last stage), then a second buffer
-        // per group if there is room
         g = gthr < bmax ? gthr : bmax;
-        if (g < 1) g = 1;
-        nbg = bmax / g >= 2 ? 2 : 1;
-        if (plan->opt_ring > 0) nbg = plan->opt_ring;
-        if (plan->opt_groups > 0) g = plan->opt_groups;
-        while (g > 1 && (g * GT > cap || g * nbg > bmax)) --g;
-        while (nbg > 1 && g * nbg > bmax) --nbg;
+        if (plan->opt_groups > 0 && plan->opt_groups < g) g = plan->opt_groups;
         if (g > tiles_per_cta) g = (int)(tiles_per_cta > 0 ? tiles_per_cta : 1);
         if (g < 1) g = 1;
     }
-    while (nbg > 1 && nbg * g > bmax) --nbg;
-    if (nbg > 4) nbg = 4;
+    // measured (configs 2a, 3, 4, 5): the contiguous-axis passes are fastest without spare buffers
+    int nb = g;
+    if (plan->opt_ring > 0) nb = plan->opt_ring < bmax ? plan->opt_ring : bmax;
+    if (nb < g) nb = g;
+    if (nb > 12) nb = 12;
     *G = g;
-    *NBG = nbg;
+    *NB = nb;
 }
 
 // contiguous-axis pass of a 2D/3D lattice through the ring pipeline (sso_ring.cuh).  `row` selects the field
@@ -1143,13 +1149,12 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     const long long ntiles = lines * plan->ncomp / TL;
     if (ntiles > 0x7fffffffLL) return fail(plan, SSO_ERR_UNSUPPORTED, "too many tiles");
     // G groups, each with its own NBG buffers (NBG = 2: the next tile loads while the current one is worked on)
-    const size_t avail = (size_t)plan->smem_optin - 256 - twbytes;
+    const size_t avail = (size_t)plan->smem_optin - 512 - twbytes;
     const int bmax = (int)(avail / bufbytes);
     if (bmax < 1) return fail(plan, SSO_ERR_UNSUPPORTED, "line too long for the ring pipeline");
-    int G = 1, NBG = 1;
-    choose_groups(plan, GT, bmax, (ntiles + plan->num_sms - 1) / plan->num_sms, &G, &NBG);
+    int G = 1, NB = 1;
+    choose_groups(plan, GT, bmax, (ntiles + plan->num_sms - 1) / plan->num_sms, &G, &NB);
     const int maxt = plan->opt_maxt ? plan->opt_maxt : (G * GT <= 384 ? 384 : 512);
-    const int NB = G * NBG;
     RingArgs a{};
     a.psi = psi;
     a.tw = A.tw;
@@ -1165,6 +1170,8 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     a.ncomp = plan->ncomp;
     const Geometry g = geometry(plan, last);
     a.rest1 = g.rest1;
+    a.rest1_shift = ilog2ll(g.rest1);
+    a.ncomp_shift = ilog2ll(plan->ncomp);
     a.vtab = mode == MODE_MID ? plan->d_vfull : plan->d_vtab;
     a.vrep = plan->vrep;
     a.rev = tile_order_mask(plan) & 1;
@@ -1175,7 +1182,7 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     }
     RingLaunchFn fn = find_ring(plan->precision, A.n, mode, maxt);
     if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no ring kernel built for this line length");
-    const size_t smem = twbytes + (size_t)NB * bufbytes + (size_t)NB * 8 + (size_t)(NB + 1) * 4;
+    const size_t smem = twbytes + (size_t)NB * bufbytes + ring_state_bytes(NB, G);
     const unsigned grid = (unsigned)(ntiles < plan->num_sms ? ntiles : plan->num_sms);
     cudaError_t e = fn(a, (unsigned)(G * GT), smem, grid, st);
     return pass_status(plan, mode == MODE_OPEN ? "ring opening pass" : (mode == MODE_MID ? "ring potential pass" : "ring closing pass"), e);
@@ -1214,10 +1221,10 @@ SRingShape sring_shape(const sso_plan *plan, int axis, int cc, bool light) {
     const Geometry g = geometry(plan, axis);
     const int U = A.n / 16, esz = (int)plan->esize();
     const int Gn = 128 / esz;  // complex numbers per 128 bytes
-    // twiddles + the pass's line table come first in shared memory; 256 bytes hold the pool's barriers and mailboxes
+    // twiddles + the pass's line table come first in shared memory; 512 bytes hold the pool's barriers, slots and mailboxes
     const size_t tw = (size_t)twiddle_count_padded(A.n) * esz + (size_t)sring_line_table_bytes(smode, A.n, esz);
-    if (tw + 256 >= plan->smem_optin) return r;
-    const size_t room = plan->smem_optin - 256 - tw;
+    if (tw + 512 >= plan->smem_optin) return r;
+    const size_t room = plan->smem_optin - 512 - tw;
     auto pitch_of = [&](int TL) { return A.n + A.n / 16 + (Gn / TL > 1 ? Gn / TL : 1); };
     auto bufbytes_of = [&](int TL) { return ((size_t)cc * TL * pitch_of(TL) * esz + 127) & ~(size_t)127; };
     // a tile shape is usable when whole warps make a group, a row is at least 16 bytes, and the cc components of a
@@ -1234,8 +1241,9 @@ SRingShape sring_shape(const sso_plan *plan, int axis, int cc, bool light) {
         return true;
     };
     int TL = 0, bm = 0;
-    if (plan->opt_tl_strided > 0) {
-        if (fits(plan->opt_tl_strided, &bm)) TL = plan->opt_tl_strided;
+    const int want_tl = light ? plan->opt_tl_middle : plan->opt_tl_strided;
+    if (want_tl > 0) {
+        if (fits(want_tl, &bm)) TL = want_tl;
     } else {
         // the widest rows (up to 128 bytes) that leave room for two buffers or more
         for (int want = 2; want >= 1 && !TL; --want)
@@ -1264,7 +1272,7 @@ SRingShape sring_shape(const sso_plan *plan, int axis, int cc, bool light) {
     if (G < 1) G = 1;
     int NB = light ? G : bmax;
     if (NB > 2 * G) NB = 2 * G;
-    if (plan->opt_ring > 0 && plan->opt_ring < NB) NB = plan->opt_ring;
+    if (plan->opt_ring > 0) NB = plan->opt_ring < bmax ? plan->opt_ring : bmax;
     if (NB < G) NB = G;
     r.G = G;
     r.NB = NB;
@@ -1307,6 +1315,8 @@ int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long 
     a.tiles_per_outer = (int)(g.inner / sh.TL);
     a.box_rows = sh.box_rows;
     a.rest1 = g.rest1;
+    a.rest1_shift = ilog2ll(g.rest1);
+    a.tpo_shift = ilog2ll(a.tiles_per_outer);
     const long long outer = plan->npts / (A.n * g.inner);
     const long long ntiles = (cc == 1 ? outer * plan->ncomp : 1) * a.tiles_per_outer;
     if (ntiles > 0x7fffffffLL) return fail(plan, SSO_ERR_UNSUPPORTED, "too many tiles");
@@ -1342,7 +1352,7 @@ int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long 
     }
     SRingLaunchFn fn = find_sring(plan->precision, A.n, smode);
     if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no strided ring kernel built for this line length");
-    const size_t smem = sh.twbytes + (size_t)sh.NB * sh.bufbytes + (size_t)sh.NB * 12 + 4;
+    const size_t smem = sh.twbytes + (size_t)sh.NB * sh.bufbytes + ring_state_bytes(sh.NB, sh.G);
     const unsigned grid = (unsigned)(ntiles < plan->num_sms ? ntiles : plan->num_sms);
     cudaError_t e = fn(a, &plan->tmap[axis], (unsigned)(a.G * sh.GT), smem, grid, st);
     return pass_status(plan, smode == SMODE_DIF ? "strided ring DIF pass" : (smode == SMODE_DIT ? "strided ring DIT pass" : "strided ring kinetic pass"), e);

@@ -84,6 +84,7 @@ struct RingArgs {
     int ncomp;                // components; tile index = line block * ncomp + component, so that the tiles that share
                               // a potential-table block run at the same time and the block is fetched from HBM once
     int rest1;                // table line = ia * rest1 + ib
+    int rest1_shift, ncomp_shift;  // log2 of rest1 and ncomp (lattice sizes are powers of two)
     const void *vtab;         // MODE_MID: merged phase exp(-i V tau), permuted slots; else exp(-i V tau/2), natural
     int vrep;                 // VREP_TABLE (complex phases) or VREP_ANGLE (real angles, sincos in the kernel)
     const void *eline;        // complex[N] field phase along the line for this pass (same order as vtab) or NULL
@@ -108,6 +109,7 @@ struct SRingArgs {
     int tiles_per_outer;      // inner / TL
     int box_rows;             // rows per TMA box (<= 256); a tile is CC * N / box_rows boxes
     int rest1;                // line = ia * rest1 + ib on the non-line axes
+    int rest1_shift, tpo_shift;  // log2 of rest1 and tiles_per_outer (lattice sizes are powers of two)
     // kinetic factor (step-dependent shifts are resolved on the host)
     const void *kph0, *kph1, *kph2;  // Schroedinger phase tables (PassArgs)
     const double *kv0, *kv1, *kv2;   // Dirac k grids (PassArgs)

@@ -91,47 +91,69 @@ __device__ __forceinline__ void prefetch_l2_bulk_plain(const void *p, unsigned b
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
-// Tile buffers of a persistent CTA: NB shared-memory buffers, G compute groups, buffer b owned by group b mod G
-// (so a group owns NB / G buffers, the first NB mod G groups one more).  A group's leader fills its buffers, its
-// threads consume them in turn, so a buffer's mbarrier never sees a waiter that is not in step with its fills
-// (a ring shared between groups let a fast group wait on a buffer one fill ahead of its phase, and an in-order
-// shared queue made fast groups wait for slow ones).  Which tile a buffer gets next is decided when the buffer is
-// refilled, from a counter shared by the CTA: the tiles are spread evenly whatever their count, and a group with
-// more buffers simply works through more tiles.
+// Tile buffers of a persistent CTA: NB shared-memory buffers shared by G compute groups (NB >= G).  The CTA's tiles
+// 0 .. nloc-1 are loaded in that order, each into whichever buffer is free: the first NB go to buffers 0 .. NB-1,
+// and every time a group has emptied a buffer its leader claims the next unloaded tile for it.  Groups consume the
+// tiles in the same order: a leader draws a ticket s (= the s-th tile of the CTA) from a counter, looks up which
+// buffer that tile went to, and the group waits for it there.  With NB > G the spare buffers hold tiles that are
+// loading or ready while all groups compute, so a group that finishes finds its next tile already on chip; with
+// NB = G a group simply gets back the buffer it refilled.
+// A waiter cannot be a fill ahead of its barrier's phase: the slot of tile s names the buffer AND the parity of the
+// fill, and it is published only when that fill is issued, i.e. after the buffer's previous fill has been consumed.
+// (A fixed ticket -> buffer map does not have that property: a group can lap a slow one and wait on a buffer whose
+// previous fill has not even landed, and the parity of its wait then matches a phase that is two fills old.)
 struct TileRing {
+    static constexpr int QN = 32;  // slots in flight: more than NB + G
     unsigned long long *bar;  // [NB] "tile landed" barriers
-    volatile int *kt;         // [NB] tile held by each buffer, -1: none left
-    int *next;                // next unclaimed tile of the CTA
+    volatile int *slot;       // [QN] slot[s % QN] = (s + 1) << 8 | parity << 7 | buffer, written when tile s is issued
+    volatile int *fills;      // [NB] fills issued into each buffer so far
+    int *next;                // next unloaded tile of the CTA
+    int *ticket;              // next ticket
+    volatile int *mail;       // [G] the ticket each group works on next
     int NB, G;
     __device__ TileRing(void *base, int nb, int g) : NB(nb), G(g) {
         bar = reinterpret_cast<unsigned long long *>(base);
-        kt = reinterpret_cast<volatile int *>(bar + nb);
-        next = const_cast<int *>(kt + nb);
+        slot = reinterpret_cast<volatile int *>(bar + nb);
+        fills = slot + QN;
+        next = const_cast<int *>(fills) + nb;
+        ticket = next + 1;
+        mail = ticket + 1;
     }
-    static __host__ __device__ size_t bytes(int nb) { return (size_t)nb * 12 + 4; }
+    static __host__ __device__ size_t bytes(int nb, int g) { return (size_t)nb * 12 + QN * 4 + 8 + (size_t)g * 4; }
     __device__ void *full(int b) const { return bar + b; }
     // once per CTA, by thread 0, before the __syncthreads that precedes the first fill
     __device__ void init() const {
         if (threadIdx.x == 0) {
-            for (int b = 0; b < NB; ++b) mbar_init(bar + b, 1);
+            for (int b = 0; b < NB; ++b) {
+                mbar_init(bar + b, 1);
+                fills[b] = 0;
+            }
+            for (int q = 0; q < QN; ++q) slot[q] = 0;
             *next = NB;  // tiles 0 .. NB-1 go to buffers 0 .. NB-1
+            *ticket = 0;
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
     }
-    __device__ int owned(int grp) const { return (NB - grp + G - 1) / G; }            // buffers of this group
-    __device__ int buffer(int grp, int j) const { return grp + G * (j % owned(grp)); }  // buffer of its j-th tile
-    // blocks until the group's j-th fill has landed; returns the tile (-1: no tiles left)
-    __device__ int wait(int grp, int j) const {
-        const int nb = owned(grp), b = grp + G * (j % nb);
-        mbar_wait(bar + b, (unsigned)((j / nb) & 1));
-        return kt[b];
+    // by the thread that issues the load of tile s into buffer b (one issuer per buffer at a time): publish where
+    // tile s lands; the caller arms the barrier and starts the copy
+    __device__ void publish(int s, int b) const {
+        const int f = fills[b];
+        fills[b] = f + 1;
+        const int par = f & 1;
+        slot[s % QN] = ((s + 1) << 8) | (par << 7) | b;
+    }
+    // group leader: draw the group's next ticket; the group barrier that follows publishes it
+    __device__ void draw(int grp) const { mail[grp] = atomicAdd(ticket, 1); }
+    __device__ int drawn(int grp) const { return mail[grp]; }
+    // blocks until tile s (< nloc) has landed; returns its buffer
+    __device__ int wait(int s) const {
+        int v;
+        while (((v = slot[s % QN]) >> 8) != s + 1) __nanosleep(64);
+        const int b = v & 127;
+        mbar_wait(bar + b, (unsigned)((v >> 7) & 1));
+        return b;
     }
     __device__ int claim() const { return atomicAdd(next, 1); }
-    // a buffer with no tile left completes its phase by hand so that its group sees the end
-    __device__ void mark(int b, int k, int nloc) const {
-        kt[b] = k < nloc ? k : -1;
-        if (k >= nloc) mbar_arrive(bar + b);
-    }
 };
 
 template <typename T, int N, int MODE, int SIGN, int MAXT>
@@ -145,10 +167,7 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     C *stw = reinterpret_cast<C *>(smem_raw);
     C *bufs = stw + TWP;
-    unsigned long long *full = reinterpret_cast<unsigned long long *>(bufs + (size_t)a.NB * a.bufstride);
-    // ktile[b] = CTA-local tile held by buffer b (-1: none left); ktile[NB] = next unclaimed local tile.  Groups
-    // claim tiles as they finish, so a CTA's tiles are shared evenly even when their count is no multiple of G
-    volatile int *ktile = reinterpret_cast<volatile int *>(full + a.NB);
+    TileRing ring(bufs + (size_t)a.NB * a.bufstride, a.NB, a.G);
 
     const int TL = a.TL, GT = a.GT, G = a.G, NB = a.NB;
     const int grp = threadIdx.x / GT;
@@ -167,7 +186,7 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     // issue the load of local tile k into its ring buffer, and ask L2 for that tile's potential-phase lines
     // tile -> first element of psi and first potential-table line (component fastest)
     auto tile_elem = [&](long long tile, long long *table_line) {
-        const long long comp = tile % a.ncomp, lb = tile / a.ncomp;
+        const long long comp = tile & (a.ncomp - 1), lb = tile >> a.ncomp_shift;  // ncomp is 1, 2 or 4
         *table_line = lb * TL;
         return (comp * a.lines_per_comp + lb * TL) * (long long)N;
     };
@@ -181,19 +200,15 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
         const long long tile = tile_of(k);
         long long l0;
         const long long e0 = tile_elem(tile, &l0);
-        mbar_expect_tx(&full[b], tile_bytes);
-        bulk_load(bufs + (size_t)b * a.bufstride, gpsi + e0, tile_bytes, &full[b]);
-        if (a.vtab && tile % a.ncomp == 0)  // one request per table block
+        mbar_expect_tx(ring.full(b), tile_bytes);
+        bulk_load(bufs + (size_t)b * a.bufstride, gpsi + e0, tile_bytes, ring.full(b));
+        if (a.vtab && (tile & (a.ncomp - 1)) == 0)  // one request per table block
             prefetch_l2_bulk_plain(reinterpret_cast<const char *>(a.vtab) + (size_t)l0 * N * vesz, (unsigned)(TL * N * vesz));
     };
 
     // let the next pass of the stream start its own setup as SMs free up
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    if (threadIdx.x == 0) {
-        ktile[NB] = NB;
-        for (int b = 0; b < NB; ++b) mbar_init(&full[b], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
+    ring.init();
     {
         const C *__restrict__ gtw = reinterpret_cast<const C *>(a.tw);
         for (int i = threadIdx.x; i < TWN; i += blockDim.x) stw[i] = gtw[i];
@@ -201,27 +216,23 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     __syncthreads();
     // everything above touched only plan-owned tables; psi is valid once the previous pass has completed
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    // every group owns NBG = NB / G buffers: its leader fills them, its threads consume them, so a buffer's
-    // mbarrier never sees a waiter that is not in step with its fills
-    const int NBG = NB / G;
-    // hand a buffer its next tile: load it, or mark the buffer empty and complete its phase by hand
+    // hand a buffer its next tile, if there is one left
     auto refill = [&](int kn, int b) {
         if (kn < nloc) {
-            ktile[b] = kn;
+            ring.publish(kn, b);
             issue(kn, b);
-        } else {
-            ktile[b] = -1;
-            mbar_arrive(&full[b]);
         }
     };
-    if (tid == 0)
-        for (int j = 0; j < NBG; ++j) refill(grp * NBG + j, grp * NBG + j);
+    if (tid == 0) {
+        for (int b = grp; b < NB; b += G) refill(b, b);  // the first NB tiles, loaded by the groups' leaders
+        ring.draw(grp);
+    }
+    gsync(gb);  // publishes the group's first ticket
 
-    for (int j = 0;; ++j) {
-        const int b = grp * NBG + j % NBG;
-        mbar_wait(&full[b], (unsigned)((j / NBG) & 1));
-        const int k = ktile[b];
-        if (k < 0) break;
+    for (;;) {
+        const int k = ring.drawn(grp);  // the group's next tile, in the CTA's loading order
+        if (k >= nloc) break;
+        const int b = ring.wait(k);
         C *buf = bufs + (size_t)b * a.bufstride;
         C *dense = buf + t * N + u;          // bulk-copy layout: [TL][N]
         C *sl = buf + t * a.pitch;           // exchange layout: padded lines
@@ -246,11 +257,11 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
             C s = mk<C>((T)1, (T)0);
             bool has_s = false;
             if (a.eoA) {
-                s = reinterpret_cast<const C *>(a.eoA)[lic / a.rest1];
+                s = reinterpret_cast<const C *>(a.eoA)[lic >> a.rest1_shift];
                 has_s = true;
             }
             if (a.eoB) {
-                const C sb = reinterpret_cast<const C *>(a.eoB)[lic % a.rest1];
+                const C sb = reinterpret_cast<const C *>(a.eoB)[lic & (a.rest1 - 1)];
                 s = has_s ? cmul(s, sb) : sb;
                 has_s = true;
             }
@@ -316,8 +327,9 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
         // the buffer was written with ordinary (generic-proxy) stores and is refilled by the bulk-copy engine (async
         // proxy): every thread orders its accesses before the refill, then the group meets
         fence_async_smem();
+        if (tid == 0) ring.draw(grp);  // the group's next ticket, published by the barrier
         gsync(gb);  // every thread of the group is done with the buffer: it can take its next tile right away
-        if (tid == 0) refill(atomicAdd(const_cast<int *>(&ktile[NB]), 1), b);
+        if (tid == 0) refill(ring.claim(), b);
         // results go straight from registers to global memory (512 contiguous bytes per warp instruction):
         // no second trip through shared memory and nothing to wait for before the buffer is refilled
         {

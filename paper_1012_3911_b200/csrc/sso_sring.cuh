@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
     };
     auto issue = [&](int k, int b) {
         const int tile = tile_of(k);
-        const int o = tile / a.tiles_per_outer, i0 = (tile % a.tiles_per_outer) * TL;
+        const int o = tile >> a.tpo_shift, i0 = (tile & (a.tiles_per_outer - 1)) * TL;  // lattice sizes are powers of two
         C *dst = bufs + (size_t)b * a.bufstride;
         mbar_expect_tx(ring.full(b), tile_bytes);
         for (int cc = 0; cc < CC; ++cc)
@@ -187,11 +187,15 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
     // everything above touched only plan-owned tables; psi is valid once the previous pass has completed
     asm volatile("griddepcontrol.wait;" ::: "memory");
     auto refill = [&](int k, int b) {
-        ring.mark(b, k, nloc);
-        if (k < nloc) issue(k, b);
+        if (k < nloc) {
+            ring.publish(k, b);
+            issue(k, b);
+        }
     };
-    if (tid == 0)
-        for (int j = 0; j < ring.owned(grp); ++j) refill(grp + G * j, grp + G * j);
+    if (tid == 0) {
+        for (int b = grp; b < a.NB; b += G) refill(b, b);  // the first NB tiles, loaded by the groups' leaders
+        ring.draw(grp);
+    }
     if constexpr (LTB > 0) {
         // (the line table may have been rebuilt for this step by the kernel before this one, hence after the wait)
         double *dst = reinterpret_cast<double *>(ltab);
@@ -206,15 +210,16 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
         __syncthreads();
     }
 
-    for (int j = 0;; ++j) {
-        const int k = ring.wait(grp, j);
-        if (k < 0) break;
-        const int b = ring.buffer(grp, j);
+    gsync(gb);  // publishes the group's first ticket
+    for (;;) {
+        const int k = ring.drawn(grp);  // the group's next tile, in the CTA's loading order
+        if (k >= nloc) break;
+        const int b = ring.wait(k);
         C *buf = bufs + (size_t)b * a.bufstride;
         C *dense = buf + (size_t)c * N * TL + t;     // TMA layout [CC][N][TL]: row r of this line at dense[r * TL]
         C *sl = buf + (c * TL + t) * a.pitch;        // exchange layout: padded lines
         const int tile = tile_of(k);
-        const int line = (tile % a.tiles_per_outer) * TL + t;  // line index on the non-line axes (within a component)
+        const int line = (tile & (a.tiles_per_outer - 1)) * TL + t;  // line index on the non-line axes (within a component)
 
         C x[16];
         if constexpr (SMODE == SMODE_DIT) {
@@ -231,10 +236,10 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
         [[maybe_unused]] double w1 = 0.0, w2 = 0.0;  // c pi_1, c pi_2 of this line (pi = k - q Abar_n, reading G16)
         [[maybe_unused]] const double mc2 = a.mass * a.clight * a.clight;
         if constexpr (CC > 1) {
-            if (a.ndim == 2) w1 = a.clight * (a.kv2[line % a.rest1] - a.sh[1]);
+            if (a.ndim == 2) w1 = a.clight * (a.kv2[line & (a.rest1 - 1)] - a.sh[1]);
             if (a.ndim == 3) {
-                w1 = a.clight * (a.kv1[line / a.rest1] - a.sh[1]);
-                w2 = a.clight * (a.kv2[line % a.rest1] - a.sh[2]);
+                w1 = a.clight * (a.kv1[line >> a.rest1_shift] - a.sh[1]);
+                w2 = a.clight * (a.kv2[line & (a.rest1 - 1)] - a.sh[2]);
             }
         }
         // per-line factor of the Schroedinger kinetic phase (the other axes' tables), requested before the forward
@@ -243,11 +248,11 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
         [[maybe_unused]] bool has_s = false;
         if constexpr (SMODE == SMODE_KS) {
             if (a.kph1) {
-                s = reinterpret_cast<const C *>(a.kph1)[line / a.rest1];
+                s = reinterpret_cast<const C *>(a.kph1)[line >> a.rest1_shift];
                 has_s = true;
             }
             if (a.kph2) {
-                const C s2 = reinterpret_cast<const C *>(a.kph2)[line % a.rest1];
+                const C s2 = reinterpret_cast<const C *>(a.kph2)[line & (a.rest1 - 1)];
                 s = has_s ? cmul(s, s2) : s2;
                 has_s = true;
             }
@@ -276,12 +281,13 @@ __global__ void __launch_bounds__(512, 1) sring_kernel(const SRingArgs a, const 
         if constexpr (SMODE != SMODE_DIF) DitChain<T, N, LAST, +1>::run(x, u, stw, sl, gb);
 
         fence_async_smem();  // generic-proxy accesses of the buffer before its refill through the async proxy
+        if (tid == 0) ring.draw(grp);  // the group's next ticket, published by the barrier
         gsync(gb);           // every thread of the group is done with the exchange layout
         // refill the buffer at once and store from registers (a warp instruction writes 32/TL rows of TL complex numbers)
         if (tid == 0) refill(ring.claim(), b);
         {
-            const long long o = tile / a.tiles_per_outer;
-            const long long i0 = (long long)(tile % a.tiles_per_outer) * TL;
+            const long long o = tile >> a.tpo_shift;
+            const long long i0 = (long long)(tile & (a.tiles_per_outer - 1)) * TL;
             C *gout = reinterpret_cast<C *>(a.psi) + (CC > 1 ? (long long)c * a.comp_stride : o * (long long)N * a.inner) + i0 + t;
             // one 64-bit multiply per thread, then pointer increments
             if constexpr (SMODE == SMODE_DIF) {

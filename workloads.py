@@ -218,6 +218,18 @@ def dirac1d(sizes=(1024,), nsteps=100, ncomp=2) -> Workload:
     return Workload("dirac1d", tuple(sizes), dx, 1e-4, ncomp, nsteps, psi, V=V)
 
 
+def dirac2d4(sizes=(1024, 1024), nsteps=128) -> Workload:
+    """2D Dirac with all FOUR components, the shape of the paper's own 2D code and benchmark (PAPER.md:115, 284, 310:
+    "Gaussian wave packets in a harmonic potential"): harmonic well, positive-energy spin-up packet, no field."""
+    rng = np.random.default_rng(SEED0 + 7)
+    dx = (0.1, 0.1)
+    X, Y = mesh(sizes, dx)
+    V = 0.5 * (X**2 + Y**2)
+    kbar = rng.uniform(-5.0, 5.0, size=2)
+    psi = dirac_packet(sizes, dx, kbar, 1.0, 4, 1.0, C_LIGHT)
+    return Workload("dirac2d_4comp", tuple(sizes), dx, 1e-4, 4, nsteps, psi, V=V, note="harmonic well, 4 components")
+
+
 def random_state(sizes, ncomp, seed, dx=None) -> np.ndarray:
     """Unstructured complex Gaussian noise, normalised: the harshest parity input (all k populated)."""
     rng = np.random.default_rng(seed)
