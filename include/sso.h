@@ -79,6 +79,8 @@ extern "C" {
 #define SSO_OPT_DIRAC_TABLE 8            /* Dirac plans without a field, ndim >= 2: 0 = cos(E tau), sin(E tau)/E of every k point
                                             evaluated in the kinetic pass, 1 = read from a table (16 bytes per k point) */
 #define SSO_OPT_LINES_PER_TILE_MIDDLE 10 /* adjacent lines per tile in the middle-axis passes of a 3D lattice (0 = auto)  */
+#define SSO_OPT_CLUSTER_1D 11            /* 1D Schroedinger steps on a thread-block cluster: 0 = auto, 1 = off (single CTA; lattices
+                                            beyond SSO_MAX_AXIS then fail), 4 or 8 = CTAs per cluster (needs sizes[0]/value in [512, 4096]) */
 #define SSO_OPT_TILE_ORDER 9              /* order in which the passes walk their tiles: 0 = auto; otherwise value - 1 is a mask of
                                             the passes that go from the highest address down (bit 0 contiguous-axis passes,
                                             1 middle-axis forward, 2 middle-axis inverse, 3 kinetic); results do not depend on it */
@@ -86,12 +88,14 @@ extern "C" {
 
 #define SSO_MIN_AXIS 16   /* smallest supported axis length                       */
 #define SSO_MAX_AXIS 4096 /* largest supported axis length (one CTA holds a line) */
+#define SSO_MAX_AXIS_1D 32768 /* 1D Schroedinger lattices (ncomp = 1, no SSO_FIELD_E, no position-space A): the line is
+                                 spread over a thread-block cluster of 8 SMs                                         */
 
 typedef struct sso_plan sso_plan; /* opaque; owned by the library */
 
 /*
  * Create a plan for a lattice of `ndim` (1..3) axes with sizes[a] points (powers
- * of two in [SSO_MIN_AXIS, SSO_MAX_AXIS]) and spacings dx[a] > 0, time step dt
+ * of two in [SSO_MIN_AXIS, SSO_MAX_AXIS]; up to SSO_MAX_AXIS_1D for ndim = 1, ncomp = 1) and spacings dx[a] > 0, time step dt
  * (finite, may be negative: the Strang step is symmetric, so -dt undoes +dt),
  * ncomp = 1 (Schroedinger), 2 (Dirac, ndim 1 or 2) or 4 (Dirac, ndim 1..3).
  * sizes and dx are host arrays, read during the call only.  Builds the radix

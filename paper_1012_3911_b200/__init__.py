@@ -21,7 +21,7 @@ OK, ERR_INVALID, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_STATE = 0, 1, 2, 3, 4
 C64, C128 = 0, 1
 FIELD_NONE, FIELD_E, FIELD_A = 0, 1, 2
 OPT_LINES_PER_TILE_CONTIG, OPT_LINES_PER_TILE_STRIDED, OPT_POTENTIAL_PHASE = 1, 2, 3
-OPT_GROUPS_PER_CTA, OPT_RING_BUFFERS, OPT_THREADS_PER_CTA, OPT_STRIDED_RING, OPT_DIRAC_TABLE, OPT_TILE_ORDER, OPT_LINES_PER_TILE_MIDDLE = 4, 5, 6, 7, 8, 9, 10
+OPT_GROUPS_PER_CTA, OPT_RING_BUFFERS, OPT_THREADS_PER_CTA, OPT_STRIDED_RING, OPT_DIRAC_TABLE, OPT_TILE_ORDER, OPT_LINES_PER_TILE_MIDDLE, OPT_CLUSTER_1D = 4, 5, 6, 7, 8, 9, 10, 11
 
 # every symbol include/sso.h declares
 SYMBOLS = (

@@ -25,6 +25,11 @@
 #include "sso_dispatch.h"
 #include "sso_line1d_args.h"
 
+// cluster size the 4096-point 1D line uses by default (0: the single-CTA kernel); chosen by measurement on B200
+#ifndef SSO_CLUSTER_AUTO_4096
+#define SSO_CLUSTER_AUTO_4096 8
+#endif
+
 namespace sso {
 
 // ---------------------------------------------------------------------------------------------
@@ -367,6 +372,17 @@ static Line1dLaunchFn find_line1d(int precision, int N) {
     return nullptr;
 }
 
+static Line1dClusterLaunchFn find_line1d_cluster(int precision, int M, int cs) {
+    switch (M) {
+#define SSO_CASE(NN) \
+    case NN:         \
+        return precision == SSO_C64 ? sso_line1d_cluster_lookup_f32_##NN(cs) : sso_line1d_cluster_lookup_f64_##NN(cs);
+        SSO_FOR_EACH_N(SSO_CASE)
+#undef SSO_CASE
+    }
+    return nullptr;
+}
+
 static RingLaunchFn find_ring(int precision, int N, int mode, int maxt) {
     switch (N) {
 #define SSO_CASE(NN) \
@@ -417,6 +433,41 @@ static int twiddle_count_padded(int N) {
     return (cnt + 7) & ~7;
 }
 
+// Twiddle blocks of an n-point line, evaluated in long double and rounded once to the plan's precision.  Stage i of
+// the radix schedule (sub-transform length NP, radix R, NI = NP/R) stores w_NP^(l k) = exp(-2 pi i l k / NP) at
+// [k-1][l], k = 1..R-1, l < NI; the last stage needs none.
+static cudaError_t upload_twiddles(int n, int precision, void **dev) {
+    std::vector<long double> twr, twi;
+    HostSched hs(n);
+    int NP = n;
+    for (int i = 0; i + 1 < hs.m; ++i) {
+        const int R = 1 << hs.lr[i], NI = NP / R;
+        for (int k = 1; k < R; ++k)
+            for (int l = 0; l < NI; ++l) {
+                const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)((long long)l * k % NP) / (long double)NP;
+                twr.push_back(cosl(ang));
+                twi.push_back(sinl(ang));
+            }
+        NP = NI;
+    }
+    if (twr.empty()) {
+        twr.push_back(1.0L);
+        twi.push_back(0.0L);
+    }
+    const size_t cnt = twr.size();
+    const size_t esz = precision == SSO_C128 ? 16 : 8;
+    cudaError_t e = cudaMalloc(dev, cnt * esz);
+    if (e != cudaSuccess) return e;
+    if (precision == SSO_C128) {
+        std::vector<double2> tw(cnt);
+        for (size_t t = 0; t < cnt; ++t) tw[t] = make_double2((double)twr[t], (double)twi[t]);
+        return cudaMemcpy(*dev, tw.data(), cnt * esz, cudaMemcpyHostToDevice);
+    }
+    std::vector<float2> tw(cnt);
+    for (size_t t = 0; t < cnt; ++t) tw[t] = make_float2((float)twr[t], (float)twi[t]);
+    return cudaMemcpy(*dev, tw.data(), cnt * esz, cudaMemcpyHostToDevice);
+}
+
 struct Axis {
     int n = 0;
     double dx = 0.0;
@@ -463,6 +514,15 @@ struct sso_plan {
     bool ktab_valid = false;  // the table is current (plans without SSO_FIELD_A only; with it it changes every step)
     int opt_dirac_table = 0;
     int opt_tile_order = 0;   // SSO_OPT_TILE_ORDER
+    int opt_cluster = 0;      // SSO_OPT_CLUSTER_1D
+    struct ClusterLine {      // tables of the cluster version of the 1D kernel, built on first use for (cs, M = N / cs)
+        int cs = 0, M = 0;
+        void *tw = nullptr;       // twiddle blocks of the M-point transform
+        void *tcl = nullptr;      // cluster twiddles [cs][cs-1][M/cs]
+        double *kv = nullptr;     // k of the frequencies k1 + cs k2, [cs][M], rows in slot order
+        void *kph = nullptr;      // kinetic phases of those frequencies
+        bool kph_valid = false;
+    } cl;
     int opt_tl_middle = 0;    // SSO_OPT_LINES_PER_TILE_MIDDLE
     int opt_tl_contig = 0, opt_tl_strided = 0, opt_groups = 0, opt_ring = 0, opt_maxt = 0, opt_sring = 0;
     int device = 0, num_sms = 0;  // the device the plan was created on, its SM count
@@ -578,8 +638,10 @@ int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double
     for (int a = 0; a < ndim; ++a) {
         if (!(dx[a] > 0.0) || !isfinite(dx[a])) return fail(nullptr, SSO_ERR_INVALID, "dx must be positive and finite");
         if (!is_pow2(sizes[a])) return fail(nullptr, SSO_ERR_INVALID, "sizes must be powers of two");
-        if (sizes[a] < SSO_MIN_AXIS || sizes[a] > SSO_MAX_AXIS)
-            return fail(nullptr, SSO_ERR_UNSUPPORTED, "axis length outside [16, 4096]");
+        // a 1D Schroedinger line may be spread over a thread-block cluster (sso_line1d_cluster.cuh)
+        const int64_t nmax = (ndim == 1 && ncomp == 1) ? SSO_MAX_AXIS_1D : SSO_MAX_AXIS;
+        if (sizes[a] < SSO_MIN_AXIS || sizes[a] > nmax)
+            return fail(nullptr, SSO_ERR_UNSUPPORTED, "axis length outside [16, 4096] (1D Schroedinger lattices: [16, 32768])");
     }
     if (ncomp > 1 && (long long)ncomp * (sizes[0] / 16) > 512)
         return fail(nullptr, SSO_ERR_UNSUPPORTED, "Dirac plans need ncomp * sizes[0] <= 8192 (all components of a line share one CTA)");
@@ -627,44 +689,7 @@ int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double
                 revBinv[f] = p / 16;
             }
         }
-        // twiddles, evaluated in long double and rounded once to the plan's precision.  Stage i of the radix
-        // schedule (sub-transform length NP, radix R, NI = NP/R) stores w_NP^(l k) = exp(-2 pi i l k / NP) at
-        // [k-1][l], k = 1..R-1, l < NI; the last stage needs none.
-        std::vector<long double> twr, twi;
-        {
-            HostSched hs(n);
-            int NP = n;
-            for (int i = 0; i + 1 < hs.m; ++i) {
-                const int R = 1 << hs.lr[i], NI = NP / R;
-                for (int k = 1; k < R; ++k)
-                    for (int l = 0; l < NI; ++l) {
-                        const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)((long long)l * k % NP) / (long double)NP;
-                        twr.push_back(cosl(ang));
-                        twi.push_back(sinl(ang));
-                    }
-                NP = NI;
-            }
-            if (twr.empty()) {
-                twr.push_back(1.0L);
-                twi.push_back(0.0L);
-            }
-        }
-        cudaError_t e;
-        if (precision == SSO_C128) {
-            std::vector<double2> tw(twr.size());
-            for (size_t t = 0; t < twr.size(); ++t) {
-                tw[t].x = (double)twr[t];
-                tw[t].y = (double)twi[t];
-            }
-            e = upload(&A.tw, tw);
-        } else {
-            std::vector<float2> tw(twr.size());
-            for (size_t t = 0; t < twr.size(); ++t) {
-                tw[t].x = (float)twr[t];
-                tw[t].y = (float)twi[t];
-            }
-            e = upload(&A.tw, tw);
-        }
+        cudaError_t e = upload_twiddles(n, precision, &A.tw);
         if (e == cudaSuccess) e = upload((void **)&A.d_revB, revB);
         if (e == cudaSuccess) e = upload((void **)&A.d_revBinv, revBinv);
         if (e == cudaSuccess) e = upload((void **)&A.d_slot_nat, A.slot_nat);
@@ -725,6 +750,10 @@ int sso_destroy(sso_plan *plan) {
     cudaFree(plan->d_sched);
     cudaFree(plan->d_hostbuf);
     cudaFree(plan->d_scratch);
+    cudaFree(plan->cl.tw);
+    cudaFree(plan->cl.tcl);
+    cudaFree(plan->cl.kv);
+    cudaFree(plan->cl.kph);
     delete plan;
     return SSO_OK;
 }
@@ -737,6 +766,7 @@ int sso_set_constants(sso_plan *plan, double mass, double c, double charge) {
     plan->clight = c;
     plan->charge = charge;
     plan->kph_valid = false;
+    plan->cl.kph_valid = false;
     plan->ktab_valid = false;
     return SSO_OK;
 }
@@ -818,7 +848,8 @@ int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nval
         plan->e_along_last = false;
         for (int a = 0; a < 3; ++a) plan->e_axis_on[a] = false;
         plan->kph_valid = false;
-    plan->ktab_valid = false;
+        plan->cl.kph_valid = false;
+        plan->ktab_valid = false;
         return SSO_OK;
     }
     if (!step_avg || nvals <= 0) return fail(plan, SSO_ERR_INVALID, "step_avg is NULL or nvals <= 0");
@@ -864,6 +895,7 @@ int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nval
         }
     }
     plan->kph_valid = false;
+    plan->cl.kph_valid = false;
     plan->ktab_valid = false;
     return SSO_OK;
 }
@@ -914,6 +946,10 @@ int sso_set_option(sso_plan *plan, int option, int64_t value) {
                 plan->d_ktab = nullptr;
             }
             plan->ktab_valid = false;
+            return SSO_OK;
+        case SSO_OPT_CLUSTER_1D:
+            if (value != 0 && value != 1 && value != 4 && value != 8) return fail(plan, SSO_ERR_INVALID, "cluster mode must be 0 (auto), 1 (off), 4 or 8 (CTAs per cluster)");
+            plan->opt_cluster = (int)value;
             return SSO_OK;
         case SSO_OPT_TILE_ORDER:
             if (value < 0 || value > 16) return fail(plan, SSO_ERR_INVALID, "tile order must be in [0, 16]");
@@ -1139,7 +1175,9 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     const int esz = (int)plan->esize();
     const long long lines = plan->npts / A.n;       // per component
     // group tile: 128 threads = 2048 points (fewer when the lattice has fewer lines)
-    int TL = plan->opt_tl_contig > 0 ? plan->opt_tl_contig : (U >= 128 ? 1 : 128 / U);
+    // group tile: 64 threads = 1024 points when a line is that short (measured on configs 3 and 5: 8 groups of 64
+    // threads beat 4 of 128: potential pass 476 -> 427 us on config 5), else one line
+    int TL = plan->opt_tl_contig > 0 ? plan->opt_tl_contig : (U >= 64 ? 1 : 64 / U);
     while (TL > 1 && (lines % TL != 0 || TL * U > 512)) TL /= 2;
     const int GT = TL * U;
     const int pitch = A.n + A.n / 16;
@@ -1245,9 +1283,10 @@ SRingShape sring_shape(const sso_plan *plan, int axis, int cc, bool light) {
     if (want_tl > 0) {
         if (fits(want_tl, &bm)) TL = want_tl;
     } else {
-        // the widest rows (up to 128 bytes) that leave room for two buffers or more
+        // the widest rows (up to 128 bytes; 256 bytes for the transform-only passes, measured 393 -> 336 us per pass
+        // on config 5) that leave room for two buffers or more
         for (int want = 2; want >= 1 && !TL; --want)
-            for (int cand = Gn; cand >= 1 && !TL; cand /= 2)
+            for (int cand = light ? 2 * Gn : Gn; cand >= 1 && !TL; cand /= 2)
                 if (fits(cand, &bm) && bm >= want) TL = cand;
     }
     if (!TL) return r;
@@ -1459,6 +1498,82 @@ int build_ktab(sso_plan *plan, long long n, cudaStream_t st) {
     return SSO_OK;
 }
 
+// ---- 1D line on a thread-block cluster (sso_line1d_cluster.cuh) ---------------------------------------------
+// cluster size for this plan's 1D steps, 0 = the single-CTA kernels
+int cluster_size_for(const sso_plan *p) {
+    if (p->ndim != 1 || p->ncomp != 1 || p->field_kind == SSO_FIELD_E || p->d_apos || p->opt_cluster == 1) return 0;
+    const int n = p->ax[0].n;
+    auto usable = [&](int cs) { return n / cs >= 512 && n / cs <= SSO_MAX_AXIS && find_line1d_cluster(p->precision, n / cs, cs) != nullptr; };
+    if (p->opt_cluster > 1) return usable(p->opt_cluster) ? p->opt_cluster : 0;
+    if (n > SSO_MAX_AXIS) return usable(8) ? 8 : (usable(4) ? 4 : 0);
+    return (n == SSO_MAX_AXIS && usable(SSO_CLUSTER_AUTO_4096)) ? SSO_CLUSTER_AUTO_4096 : 0;
+}
+
+int build_cluster_tables(sso_plan *plan, int cs) {
+    sso_plan::ClusterLine &cl = plan->cl;
+    const int N = plan->ax[0].n, M = N / cs, MC = M / cs, U = M / 16;
+    if (cl.cs == cs && cl.M == M) return SSO_OK;
+    cudaFree(cl.tw);
+    cudaFree(cl.tcl);
+    cudaFree(cl.kv);
+    cudaFree(cl.kph);
+    cl = sso_plan::ClusterLine();
+    cudaError_t e = upload_twiddles(M, plan->precision, &cl.tw);
+    // w_N^(m k1) for m = r MC + mm, stored [r][k1 - 1][mm] (eq. 12 sign), long double, rounded once
+    std::vector<double2> t64((size_t)cs * (cs - 1) * MC);
+    for (int r = 0; r < cs; ++r)
+        for (int k1 = 1; k1 < cs; ++k1)
+            for (int mm = 0; mm < MC; ++mm) {
+                const long long m = (long long)r * MC + mm;
+                const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)((m * k1) % N) / (long double)N;
+                t64[((size_t)r * (cs - 1) + (k1 - 1)) * MC + mm] = make_double2((double)cosl(ang), (double)sinl(ang));
+            }
+    if (e == cudaSuccess) {
+        if (plan->precision == SSO_C128) e = upload(&cl.tcl, t64);
+        else {
+            std::vector<float2> t32(t64.size());
+            for (size_t i = 0; i < t64.size(); ++i) t32[i] = make_float2((float)t64[i].x, (float)t64[i].y);
+            e = upload(&cl.tcl, t32);
+        }
+    }
+    // frequency held by CTA k1 at slot s of its M-point transform: k1 + cs k2, k2 = slot_nat_M[s]
+    std::vector<double> kv((size_t)N);
+    for (int p = 0; p < M; ++p) {
+        const int k2 = freq_of_pos(M, p), s = (p % 16) * U + p / 16;
+        for (int k1 = 0; k1 < cs; ++k1) kv[(size_t)k1 * M + s] = plan->ax[0].k_nat[k1 + cs * k2];
+    }
+    if (e == cudaSuccess) e = upload((void **)&cl.kv, kv);
+    if (e == cudaSuccess) e = cudaMalloc(&cl.kph, (size_t)N * plan->esize());
+    if (e != cudaSuccess) {
+        cudaFree(cl.tw);
+        cudaFree(cl.tcl);
+        cudaFree(cl.kv);
+        cudaFree(cl.kph);
+        cl = sso_plan::ClusterLine();
+        return fail(plan, SSO_ERR_ALLOC, std::string("cluster line tables: ") + cudaGetErrorString(e));
+    }
+    cl.cs = cs;
+    cl.M = M;
+    return SSO_OK;
+}
+
+// kinetic phases of the cluster layout (eq. 13), rebuilt every step with SSO_FIELD_A
+int build_kphase_cluster(sso_plan *plan, long long n, cudaStream_t st) {
+    const bool shifted = plan->field_kind == SSO_FIELD_A;
+    if (plan->cl.kph_valid && !shifted) return SSO_OK;
+    PassTimer timer(plan, SSO_PASS_TABLES, st);
+    const int N = plan->ax[0].n;
+    const int blocks = (N + 127) / 128;
+    if (plan->precision == SSO_C128)
+        build_kphase_kernel<double><<<blocks, 128, 0, st>>>(plan->cl.kv, plan->cl.kph, N, plan->dt, plan->mass, shifted ? plan->d_avg : nullptr, n, 1, 0, plan->charge, 1.0 / (double)N);
+    else
+        build_kphase_kernel<float><<<blocks, 128, 0, st>>>(plan->cl.kv, plan->cl.kph, N, plan->dt, plan->mass, shifted ? plan->d_avg : nullptr, n, 1, 0, plan->charge, 1.0 / (double)N);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(plan, e, "kinetic phase kernel (cluster layout)");
+    plan->cl.kph_valid = !shifted;
+    return SSO_OK;
+}
+
 int kinetic_pw(const sso_plan *p) { return p->ncomp == 1 ? PW_KS : (p->ncomp == 2 ? PW_KD2 : PW_KD4); }
 
 long long launches_for(const sso_plan *p, long long nsteps) {
@@ -1468,6 +1583,7 @@ long long launches_for(const sso_plan *p, long long nsteps) {
     const bool kbuild = p->ncomp == 1 && (kshift || !p->kph_valid);
     if (p->ndim == 1) {
         if (p->d_apos) return nsteps * 3;  // rotation, one step, rotation
+        if (cluster_size_for(p)) return kshift ? 2 * nsteps : 1 + (p->cl.kph_valid ? 0 : 1);
         if (kshift) return nsteps * (1 + p->ndim);
         return 1 + (kbuild ? p->ndim : 0);
     }
@@ -1515,10 +1631,32 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
         const bool kshift = plan->ncomp == 1 && plan->field_kind == SSO_FIELD_A;
         // step-dependent kinetic tables, or the position-space rotation between the steps, force one launch per step
         const long long chunk = (kshift || plan->d_apos) ? 1 : nsteps;
+        const int cs = cluster_size_for(plan);
+        if (!cs && plan->ax[0].n > SSO_MAX_AXIS)
+            return fail(plan, SSO_ERR_UNSUPPORTED, "1D lattices beyond 4096 points run on a thread-block cluster: Schroedinger without a length-gauge field only");
+        if (cs && (rc = build_cluster_tables(plan, cs)) != SSO_OK) return rc;
         for (long long s = 0; s < nsteps; s += chunk) {
+            if (chunk > 0x7fffffffLL) return fail(plan, SSO_ERR_INVALID, "nsteps too large");
+            if (cs) {
+                // the line spread over a cluster of cs CTAs, psi in registers for all steps of the launch
+                if ((rc = build_kphase_cluster(plan, n0 + s, st)) != SSO_OK) return rc;
+                PassTimer timer(plan, SSO_PASS_LINE_1D, st);
+                const int M = plan->cl.M;
+                Line1dClusterArgs la{};
+                la.psi = psi;
+                la.tw = plan->cl.tw;
+                la.tcl = plan->cl.tcl;
+                la.vtab = plan->d_vtab;
+                la.vrep = plan->vrep;
+                la.kph = plan->cl.kph;
+                la.nsteps = (int)chunk;
+                const size_t smem = ((size_t)twiddle_count_padded(M) + (M + M / 16) + (line1d_cluster_alias(M) ? 0 : M) + (size_t)(cs - 1) * (M / cs)) * plan->esize();
+                Line1dClusterLaunchFn lc = find_line1d_cluster(plan->precision, M, cs);
+                if ((rc = pass_status(plan, "1D cluster line kernel", lc(la, smem, st))) != SSO_OK) return rc;
+                continue;
+            }
             if ((rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
             if (plan->ncomp == 1 && (rc = build_kphase(plan, n0 + s, st)) != SSO_OK) return rc;
-            if (chunk > 0x7fffffffLL) return fail(plan, SSO_ERR_INVALID, "nsteps too large");
             Line1dLaunchFn l1 = (plan->ncomp == 1 && plan->field_kind != SSO_FIELD_E) ? find_line1d(plan->precision, plan->ax[0].n) : nullptr;
             if (l1) {
                 // Schroedinger without a length-gauge field: both pointwise tables are constant over the launch and

@@ -146,4 +146,13 @@ using Line1dLaunchFn = cudaError_t (*)(const Line1dArgs &, size_t smem, cudaStre
 SSO_FOR_EACH_N(SSO_DECL_LINE1D)
 #undef SSO_DECL_LINE1D
 
+// the cluster version (sso_line1d_cluster.cuh): lookup by the per-CTA length M = N / CS and the cluster size CS
+struct Line1dClusterArgs;
+using Line1dClusterLaunchFn = cudaError_t (*)(const Line1dClusterArgs &, size_t smem, cudaStream_t st);
+#define SSO_DECL_LINE1D_CL(N)                                  \
+    Line1dClusterLaunchFn sso_line1d_cluster_lookup_f32_##N(int cs); \
+    Line1dClusterLaunchFn sso_line1d_cluster_lookup_f64_##N(int cs);
+SSO_FOR_EACH_N(SSO_DECL_LINE1D_CL)
+#undef SSO_DECL_LINE1D_CL
+
 }  // namespace sso

@@ -8,6 +8,7 @@
 #include "sso_ring.cuh"
 #include "sso_sring.cuh"
 #include "sso_line1d.cuh"
+#include "sso_line1d_cluster.cuh"
 #include "sso_dispatch.h"
 
 #ifndef SSO_T
@@ -101,6 +102,27 @@ template <typename T, int N> cudaError_t launch_line1d(const Line1dArgs &a, size
     return cudaGetLastError();
 }
 
+// one cluster of CS CTAs holds the line; CS is a launch attribute (8 is the largest portable cluster size)
+template <typename T, int M, int CS> cudaError_t launch_line1d_cluster(const Line1dClusterArgs &a, size_t smem, cudaStream_t st) {
+    auto kern = line1d_cluster_kernel<T, M, CS>;
+    static std::atomic<unsigned long long> done{0};
+    cudaError_t e = opt_in_smem(kern, done);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(CS);
+    cfg.blockDim = dim3(M / 16);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = CS;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
 #define SSO_CAT3_(a, b, c) a##b##_##c
 #define SSO_CAT3(a, b, c) SSO_CAT3_(a, b, c)
 
@@ -127,6 +149,16 @@ SRingLaunchFn SSO_CAT4(sso_sring_lookup_, SSO_TNAME, SSO_N)(int mode) {
 Line1dLaunchFn SSO_CAT4(sso_line1d_lookup_, SSO_TNAME, SSO_N)() { return nullptr; }
 #else
 Line1dLaunchFn SSO_CAT4(sso_line1d_lookup_, SSO_TNAME, SSO_N)() { return &launch_line1d<SSO_T, SSO_N>; }
+#endif
+
+#if defined(SSO_STUB) || SSO_N < 512
+Line1dClusterLaunchFn SSO_CAT4(sso_line1d_cluster_lookup_, SSO_TNAME, SSO_N)(int) { return nullptr; }
+#else
+Line1dClusterLaunchFn SSO_CAT4(sso_line1d_cluster_lookup_, SSO_TNAME, SSO_N)(int cs) {
+    if (cs == 4) return &launch_line1d_cluster<SSO_T, SSO_N, 4>;
+    if (cs == 8) return &launch_line1d_cluster<SSO_T, SSO_N, 8>;
+    return nullptr;
+}
 #endif
 
 #ifdef SSO_STUB
