@@ -205,6 +205,24 @@ int sso_spectrum(sso_plan *plan, const double *chi_host, int64_t nt, double dts,
 int sso_filter_accumulate(sso_plan *plan, void *acc, const void *psi, double t, double T, double E, double dts,
                           void *stream);
 
+/*
+ * Observables FUSED INTO THE LAST PASS of a call: advances psi by nsteps >= 1 steps exactly like
+ * sso_step and returns, for the resulting psi(t),
+ *   out_host[0]      sum |psi|^2 prod(dx)                                   (the norm)
+ *   out_host[1..2]   Re, Im of <psi_ref | psi(t)>  (eq. 40; 0 when psi_ref is NULL)
+ *   out_host[3..5]   <r_a>, a < ndim (the rest 0)
+ * and, when filter_acc is not NULL, adds the term psi(t) (1 - cos(2 pi filter_t/filter_T)) exp(i filter_E filter_t)
+ * filter_dts of the eigenfunction filter (eq. 42) to the complex128 DEVICE array filter_acc
+ * (ncomp * prod(sizes) numbers, caller-owned).  On 2D/3D lattices all of it is accumulated by the closing pass of the
+ * call while the result is still in registers: psi(t) makes no extra trip through HBM (psi_ref and filter_acc are
+ * read, filter_acc written, once).  1D lattices (psi does not leave the SM during a call) and plans with a
+ * position-space vector potential use the separate kernels above after the steps; the results are the same.  The sums
+ * are accumulated in double; their last bits may differ from run to run (which tiles a warp meets is decided at run
+ * time).  psi_ref is a DEVICE array laid out like psi.  Synchronises `stream`.
+ */
+int sso_step_observe(sso_plan *plan, void *psi, int64_t nsteps, const void *psi_ref, void *filter_acc, double filter_t,
+                     double filter_T, double filter_E, double filter_dts, double *out_host, void *stream);
+
 /* Tuning knobs (SSO_OPT_*); invalid values give SSO_ERR_INVALID. */
 int sso_set_option(sso_plan *plan, int option, int64_t value);
 

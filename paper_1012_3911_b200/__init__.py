@@ -29,7 +29,7 @@ SYMBOLS = (
     "sso_get_time_index", "sso_step", "sso_step_host", "sso_norm", "sso_set_option", "sso_launch_count",
     "sso_destroy", "sso_last_error", "sso_version", "sso_debug_layout", "sso_profile_step", "sso_pass_name",
     "sso_set_vector_potential", "sso_overlap", "sso_expect_position", "sso_expect_momentum", "sso_spectrum",
-    "sso_filter_accumulate",
+    "sso_filter_accumulate", "sso_step_observe",
 )
 PASS_KINDS = 9
 
@@ -74,6 +74,7 @@ def lib() -> ctypes.CDLL:
         L.sso_expect_momentum.argtypes = [vp, vp, ctypes.POINTER(dbl), vp]
         L.sso_spectrum.argtypes = [vp, vp, i64, dbl, vp, i64, vp, vp]
         L.sso_filter_accumulate.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp]
+        L.sso_step_observe.argtypes = [vp, vp, i64, vp, vp, dbl, dbl, dbl, dbl, ctypes.POINTER(dbl), vp]
         L.sso_pass_name.restype = ctypes.c_char_p
         for name in SYMBOLS:
             if name not in ("sso_last_error", "sso_version", "sso_pass_name"):
@@ -238,6 +239,17 @@ class Plan:
         _check_buffer(acc, self._npts * self.ncomp * 16, 16, True, "acc")
         _check_buffer(psi, self._psi_bytes, self._esz, True, "psi")
         self._ck(lib().sso_filter_accumulate(self._h, _ptr(acc), _ptr(psi), float(t), float(T), float(E), float(dts), _stream(stream)))
+
+    def step_observe(self, psi, nsteps: int, psi_ref=None, filter_acc=None, filter_t: float = 0.0, filter_T: float = 1.0,
+                     filter_E: float = 0.0, filter_dts: float = 0.0, stream=None):
+        """sso_step_observe: step, and return (norm, <psi_ref|psi>, [<r_a>]) of the result from the closing pass."""
+        _check_buffer(psi, self._psi_bytes, self._esz, True, "psi")
+        _check_buffer(psi_ref, self._psi_bytes, self._esz, True, "psi_ref")
+        _check_buffer(filter_acc, self._npts * self.ncomp * 16, 16, True, "filter_acc")
+        out = (ctypes.c_double * 6)()
+        self._ck(lib().sso_step_observe(self._h, _ptr(psi), int(nsteps), _ptr(psi_ref), _ptr(filter_acc), float(filter_t), float(filter_T),
+                                        float(filter_E), float(filter_dts), out, _stream(stream)))
+        return out[0], complex(out[1], out[2]), [out[3 + a] for a in range(len(self.sizes))]
 
     def profile_step(self, psi, nsteps: int, stream=None):
         """sso_profile_step: [(pass name, launches, mean microseconds)] for the pass kinds that ran."""

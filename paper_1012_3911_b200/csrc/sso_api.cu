@@ -709,7 +709,7 @@ int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double
         }
     }
     cudaError_t e = cudaMalloc((void **)&plan->d_partial, sizeof(double) * 4 * NORM_BLOCKS);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&plan->d_norm, sizeof(double) * 4);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&plan->d_norm, sizeof(double) * 8);
     if (e == cudaSuccess) e = cudaMalloc((void **)&plan->d_sched, 2 * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMemset(plan->d_sched, 0, 2 * sizeof(unsigned));
     if (e != cudaSuccess) {
@@ -1019,8 +1019,8 @@ int tile_order_mask(const sso_plan *p) {
     return p->ndim == 3 ? 1 : 0;
 }
 
-// shared-memory bytes of a pass's buffer pool state (sso_ring.cuh, TileRing::bytes): barriers, tiles, counters, mailboxes
-size_t ring_state_bytes(int nb, int g) { return (size_t)nb * 12 + 32 * 4 + 8 + (size_t)g * 4; }
+// Every ring pass reserves 512 bytes of shared memory behind its buffers: the pool state of sso_ring.cuh (TileRing::bytes:
+// 12 NB + 136 + 4 G <= 340 for NB <= 12, G <= 15) and, from byte 448, the observable sums of the closing pass.
 
 // lines per component per CTA
 int choose_tl(const sso_plan *p, const Geometry &g, int cc) {
@@ -1165,9 +1165,17 @@ void choose_groups(const sso_plan *plan, int GT, int bmax, long long tiles_per_c
     *NB = nb;
 }
 
+// observables asked of the closing pass of a call (sso_step_observe)
+struct ObsRequest {
+    const void *ref;
+    void *facc;
+    double t, T, E, dts;
+    int grid;  // CTAs of the closing pass that wrote partial sums (set by launch_ring_pass)
+};
+
 // contiguous-axis pass of a 2D/3D lattice through the ring pipeline (sso_ring.cuh).  `row` selects the field
 // phase row of this call (build_erows_kernel): 0 opening, j merged after step j-1, nsteps closing.
-int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStream_t st) {
+int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStream_t st, ObsRequest *obs = nullptr) {
     PassTimer timer(plan, mode == MODE_OPEN ? SSO_PASS_OPENING : (mode == MODE_MID ? SSO_PASS_POTENTIAL : SSO_PASS_CLOSING), st);
     const int last = plan->ndim - 1;
     const Axis &A = plan->ax[last];
@@ -1218,10 +1226,29 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
         if (g.oaxA >= 0 && plan->e_axis_on[g.oaxA]) a.eoA = (const char *)plan->d_erow[g.oaxA] + (size_t)row * plan->ax[g.oaxA].n * esz;
         if (g.oaxB >= 0 && plan->e_axis_on[g.oaxB]) a.eoB = (const char *)plan->d_erow[g.oaxB] + (size_t)row * plan->ax[g.oaxB].n * esz;
     }
+    const unsigned grid = (unsigned)(ntiles < plan->num_sms ? ntiles : plan->num_sms);
+    if (obs) {
+        mode = MODE_CLOSE_OBS;
+        a.ref = obs->ref;
+        a.facc = obs->facc;
+        a.fw_t = obs->t;
+        a.fw_T = obs->T;
+        a.fw_E = obs->E;
+        a.fw_dts = obs->dts;
+        a.obs_partial = plan->d_partial;
+        a.obs_axA = g.oaxA;
+        a.obs_axB = g.oaxB;
+        a.obs_axL = last;
+        const int axs[3] = {g.oaxA, g.oaxB, last};
+        for (int i = 0; i < 3; ++i) {
+            a.obs_dx[i] = axs[i] >= 0 ? plan->ax[axs[i]].dx : 0.0;
+            a.obs_half[i] = axs[i] >= 0 ? plan->ax[axs[i]].n / 2 : 0;
+        }
+        obs->grid = (int)grid;
+    }
     RingLaunchFn fn = find_ring(plan->precision, A.n, mode, maxt);
     if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no ring kernel built for this line length");
-    const size_t smem = twbytes + (size_t)NB * bufbytes + ring_state_bytes(NB, G);
-    const unsigned grid = (unsigned)(ntiles < plan->num_sms ? ntiles : plan->num_sms);
+    const size_t smem = twbytes + (size_t)NB * bufbytes + 512;  // pool state (ring_state_bytes <= 400) + observable scratch
     cudaError_t e = fn(a, (unsigned)(G * GT), smem, grid, st);
     return pass_status(plan, mode == MODE_OPEN ? "ring opening pass" : (mode == MODE_MID ? "ring potential pass" : "ring closing pass"), e);
 }
@@ -1391,7 +1418,7 @@ int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long 
     }
     SRingLaunchFn fn = find_sring(plan->precision, A.n, smode);
     if (!fn) return fail(plan, SSO_ERR_UNSUPPORTED, "no strided ring kernel built for this line length");
-    const size_t smem = sh.twbytes + (size_t)sh.NB * sh.bufbytes + ring_state_bytes(sh.NB, sh.G);
+    const size_t smem = sh.twbytes + (size_t)sh.NB * sh.bufbytes + 512;
     const unsigned grid = (unsigned)(ntiles < plan->num_sms ? ntiles : plan->num_sms);
     cudaError_t e = fn(a, &plan->tmap[axis], (unsigned)(a.G * sh.GT), smem, grid, st);
     return pass_status(plan, smode == SMODE_DIF ? "strided ring DIF pass" : (smode == SMODE_DIT ? "strided ring DIT pass" : "strided ring kinetic pass"), e);
@@ -1611,7 +1638,9 @@ int sso_launch_count(const sso_plan *plan, int64_t nsteps, int64_t *count) {
     return SSO_OK;
 }
 
-int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
+// the steps of sso_step; obs != NULL: the closing pass of the call also accumulates the observables (2D/3D lattices
+// without the position-space vector potential; *fused tells the caller whether it did)
+static int step_impl(sso_plan *plan, void *psi, int64_t nsteps, void *stream, ObsRequest *obs, bool *fused) {
     if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
     if (!psi) return fail(plan, SSO_ERR_INVALID, "psi is NULL");
     if (((uintptr_t)psi & 15u) != 0) return fail(plan, SSO_ERR_INVALID, "psi must be 16-byte aligned");
@@ -1719,7 +1748,10 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
                     if (rc != SSO_OK) return rc;
                 }
                 // F_last^-1 V(n, n+1) F_last, or the closing F_last^-1, V/2
-                if ((rc = launch_ring_pass(plan, psi, s + 1 < ns ? MODE_MID : MODE_CLOSE, s + 1, st)) != SSO_OK) return rc;
+                const bool last_of_call = s + 1 == ns && c0 + ns == nsteps;
+                ObsRequest *ob = (obs && last_of_call && !plan->d_apos) ? obs : nullptr;
+                if (ob && fused) *fused = true;
+                if ((rc = launch_ring_pass(plan, psi, s + 1 < ns ? MODE_MID : MODE_CLOSE, s + 1, st, ob)) != SSO_OK) return rc;
             }
             if ((rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
         }
@@ -1727,6 +1759,8 @@ int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) {
     plan->tindex += nsteps;
     return SSO_OK;
 }
+
+int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream) { return step_impl(plan, psi, nsteps, stream, nullptr, nullptr); }
 
 int sso_profile_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream, int64_t *count, double *mean_us) {
     if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
@@ -1908,6 +1942,37 @@ int sso_filter_accumulate(sso_plan *plan, void *acc, const void *psi, double t, 
     if (plan->precision == SSO_C128) filter_accumulate_kernel<double><<<blocks, 256, 0, st>>>(reinterpret_cast<double2 *>(acc), psi, count, t, T, E, dts);
     else filter_accumulate_kernel<float><<<blocks, 256, 0, st>>>(reinterpret_cast<double2 *>(acc), psi, count, t, T, E, dts);
     CK(cudaGetLastError());
+    return SSO_OK;
+}
+
+int sso_step_observe(sso_plan *plan, void *psi, int64_t nsteps, const void *psi_ref, void *filter_acc, double filter_t, double filter_T,
+                     double filter_E, double filter_dts, double *out_host, void *stream) {
+    if (!plan) return fail(nullptr, SSO_ERR_INVALID, "plan is NULL");
+    if (!out_host) return fail(plan, SSO_ERR_INVALID, "out_host is NULL");
+    if (nsteps < 1) return fail(plan, SSO_ERR_INVALID, "sso_step_observe needs nsteps >= 1");
+    if (filter_acc && (!(filter_T > 0.0) || !isfinite(filter_t) || !isfinite(filter_T) || !isfinite(filter_E) || !isfinite(filter_dts)))
+        return fail(plan, SSO_ERR_INVALID, "filter: T must be positive, all arguments finite");
+    cudaStream_t st = (cudaStream_t)stream;
+    ObsRequest ob{psi_ref, filter_acc, filter_t, filter_T, filter_E, filter_dts, 0};
+    bool fused = false;
+    int rc = step_impl(plan, psi, nsteps, stream, &ob, &fused);
+    if (rc != SSO_OK) return rc;
+    for (int i = 0; i < 6; ++i) out_host[i] = 0.0;
+    if (fused) {
+        double vol = 1.0;
+        for (int a = 0; a < plan->ndim; ++a) vol *= plan->ax[a].dx;
+        reduce_final_kernel<<<1, 192, 0, st>>>(plan->d_partial, ob.grid, 6, vol, plan->d_norm);
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(out_host, plan->d_norm, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        return SSO_OK;
+    }
+    // 1D lattices (psi never leaves the SM during a call) and plans with the position-space vector potential (its
+    // rotation follows the closing pass): the same quantities by the kernels of their own
+    if ((rc = sso_norm(plan, psi, &out_host[0], stream)) != SSO_OK) return rc;
+    if (psi_ref && (rc = sso_overlap(plan, psi_ref, psi, &out_host[1], stream)) != SSO_OK) return rc;
+    if ((rc = sso_expect_position(plan, psi, &out_host[3], stream)) != SSO_OK) return rc;
+    if (filter_acc && (rc = sso_filter_accumulate(plan, filter_acc, psi, filter_t, filter_T, filter_E, filter_dts, stream)) != SSO_OK) return rc;
     return SSO_OK;
 }
 

@@ -68,7 +68,7 @@ SSO_FOR_EACH_N(SSO_DECL_LOOKUP)
 #undef SSO_DECL_LOOKUP
 
 // the ring pipeline of sso_ring.cuh (contiguous-axis passes of 2D/3D lattices)
-enum : int { MODE_OPEN = 0, MODE_MID = 1, MODE_CLOSE = 2 };
+enum : int { MODE_OPEN = 0, MODE_MID = 1, MODE_CLOSE = 2, MODE_CLOSE_OBS = 3 };  // CLOSE_OBS: closing pass + observables
 
 struct RingArgs {
     void *psi;                // device, all components: ntiles * TL lines of N points, contiguous
@@ -90,6 +90,14 @@ struct RingArgs {
     const void *eline;        // complex[N] field phase along the line for this pass (same order as vtab) or NULL
     const void *eoA, *eoB;    // complex field phase rows of the other axes, indexed by ia / ib, or NULL
     int rev;                  // tiles in descending address order
+    // MODE_CLOSE_OBS: observables of the final psi accumulated in the closing pass
+    const void *ref;          // psi(0) for the autocorrelation function (eq. 40), laid out like psi, or NULL
+    double *obs_partial;      // [6][gridDim.x]: sum |psi|^2, Re and Im of sum conj(ref) psi, sum r_a |psi|^2 for axis a = 0, 1, 2
+    void *facc;               // complex128 accumulator of the eigenfunction filter (eq. 42), laid out like psi, or NULL
+    double fw_t, fw_T, fw_E, fw_dts;  // its term: acc += psi (1 - cos(2 pi t/T)) exp(i E t) dts
+    int obs_axA, obs_axB, obs_axL;    // lattice axes of ia, ib (-1: absent) and of the line
+    double obs_dx[3];         // dx of those three
+    int obs_half[3];          // n/2 of those three (grid of reading G14)
 };
 
 using RingLaunchFn = cudaError_t (*)(const RingArgs &, unsigned threads, size_t smem, unsigned grid, cudaStream_t st);

@@ -171,10 +171,12 @@ RingLaunchFn SSO_CAT4(sso_ring_lookup_, SSO_TNAME, SSO_N)(int mode, int maxt) {
         if (mode == MODE_OPEN) return &launch_ring<T, N, MODE_OPEN, -1, 512>;
         if (mode == MODE_MID) return &launch_ring<T, N, MODE_MID, +1, 512>;
         if (mode == MODE_CLOSE) return &launch_ring<T, N, MODE_CLOSE, +1, 512>;
+        if (mode == MODE_CLOSE_OBS) return &launch_ring<T, N, MODE_CLOSE_OBS, +1, 512>;
     } else if (maxt == 384) {
         if (mode == MODE_OPEN) return &launch_ring<T, N, MODE_OPEN, -1, 384>;
         if (mode == MODE_MID) return &launch_ring<T, N, MODE_MID, +1, 384>;
         if (mode == MODE_CLOSE) return &launch_ring<T, N, MODE_CLOSE, +1, 384>;
+        if (mode == MODE_CLOSE_OBS) return &launch_ring<T, N, MODE_CLOSE_OBS, +1, 384>;
     }
     return nullptr;
 }

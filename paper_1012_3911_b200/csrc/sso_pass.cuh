@@ -119,48 +119,66 @@ __host__ __device__ constexpr double sin16(int j) {
                   : 0.38268343236508977173;
 }
 
-// v * exp(SIGN 2 pi i j / R), j < R/2, all compile-time after unrolling
-template <int R, int SIGN, typename C> __device__ __forceinline__ C mul_root(C v, int j) {
-    using T = decltype(C::x);
-    const int j16 = j * (16 / R);
-    if (j16 == 0) return v;
-    if (j16 == 4) return SIGN > 0 ? mk<C>(-v.y, v.x) : mk<C>(v.y, -v.x);
-    const T c = (T)cos16(j16);
-    const T s = (T)(SIGN > 0 ? sin16(j16) : -sin16(j16));
-    return mk<C>(v.x * c - v.y * s, v.x * s + v.y * c);
-}
-
 __host__ __device__ constexpr int brevc(int k, int bits) {
     int r = 0;
     for (int b = 0; b < bits; ++b) r |= ((k >> b) & 1) << (bits - 1 - b);
     return r;
 }
 
-// radix-2 decimation-in-frequency recursion on x[j*S], j < R; output bit-reversed
-template <int R, int S, int SIGN, typename C> __device__ __forceinline__ void dif_rec(C *x) {
-    if constexpr (R >= 2) {
-        constexpr int H = R / 2;
-#pragma unroll
-        for (int j = 0; j < H; ++j) {
-            C a = x[j * S], b = x[(j + H) * S];
-            x[j * S] = cadd(a, b);
-            x[(j + H) * S] = mul_root<R, SIGN>(csub(a, b), j);
-        }
-        dif_rec<H, S, SIGN>(x);
-        dif_rec<H, S, SIGN>(x + H * S);
+// One radix-2 butterfly with the twiddle on the second input, fused into multiply-adds:
+//   (a, b) <- (a + w b, a - w b),   w = exp(SIGN 2 pi i j16 / 16),
+// 6 FP instructions for a general w (a + w b by four FMAs, a - w b = 2 a - (a + w b) by two more) against 8 for a
+// complex multiplication followed by an addition and a subtraction; 4 when w is 1 or +-i.
+template <int SIGN, typename C> __device__ __forceinline__ void bfly(C &a, C &b, int j16) {
+    using T = decltype(C::x);
+    if (j16 == 0) {
+        const C r = cadd(a, b), d = csub(a, b);
+        a = r;
+        b = d;
+    } else if (j16 == 4) {
+        // w = SIGN i:  w b = SIGN (-b.y, b.x)
+        const C wb = SIGN > 0 ? mk<C>(-b.y, b.x) : mk<C>(b.y, -b.x);
+        const C r = cadd(a, wb), d = csub(a, wb);
+        a = r;
+        b = d;
+    } else {
+        const T c = (T)cos16(j16);
+        const T s = (T)(SIGN > 0 ? sin16(j16) : -sin16(j16));
+        C r;
+        r.x = fma(-s, b.y, fma(c, b.x, a.x));
+        r.y = fma(s, b.x, fma(c, b.y, a.y));
+        b = mk<C>(fma((T)2, a.x, -r.x), fma((T)2, a.y, -r.y));
+        a = r;
     }
 }
 
-// y[k*S] = sum_j x[j*S] exp(SIGN 2 pi i j k / R), natural order in and out, in registers
-template <int R, int S, int SIGN, typename C> __device__ __forceinline__ void dft_reg(C *x) {
-    dif_rec<R, S, SIGN>(x);
-    if constexpr (R > 2) {
+// y[k*S] = sum_j x[j*S] exp(SIGN 2 pi i j k / R), natural order in and out, in registers: the iterative
+// decimation-in-time network on the bit-reversed view A[p] = x[brev(p) S] (register renaming, no data movement),
+// levels len = 2, 4, .., R with the butterflies above; A[k] = y_k at the end, copied back to natural order.
+// FIRST = false skips the first level (len = 2: the pairs x[k], x[k + R/2]), for callers that fuse it with
+// twiddles on the inputs.
+template <int R, int S, int SIGN, int LB, typename C> __device__ __forceinline__ void dft_levels(C *x) {
+    constexpr int B = ilog2c(R);
+    if constexpr (LB <= B) {
+        constexpr int LEN = 1 << LB, HALF = LEN / 2;
+#pragma unroll
+        for (int i = 0; i < R / LEN; ++i)
+#pragma unroll
+            for (int j = 0; j < HALF; ++j) bfly<SIGN>(x[brevc(i * LEN + j, B) * S], x[brevc(i * LEN + j + HALF, B) * S], j * (16 / LEN));
+        dft_levels<R, S, SIGN, LB + 1>(x);
+    }
+}
+template <int R, int S, int SIGN, typename C, bool FIRST = true> __device__ __forceinline__ void dft_reg(C *x) {
+    if constexpr (R >= 2) {
         constexpr int B = ilog2c(R);
-        C t[R];
+        dft_levels<R, S, SIGN, FIRST ? 1 : 2>(x);
+        if constexpr (R > 2) {
+            C t[R];
 #pragma unroll
-        for (int k = 0; k < R; ++k) t[k] = x[brevc(k, B) * S];
+            for (int k = 0; k < R; ++k) t[k] = x[brevc(k, B) * S];
 #pragma unroll
-        for (int k = 0; k < R; ++k) x[k * S] = t[k];
+            for (int k = 0; k < R; ++k) x[k * S] = t[k];
+        }
     }
 }
 
@@ -214,19 +232,35 @@ template <typename T, int N, int I, int SIGN> __device__ __forceinline__ void di
     constexpr int Mi = NP / 16;
     constexpr int S = 16 / R;
     if constexpr (NP > R) {
-        constexpr int NI = NP / R;
+        // the twiddles on the inputs are fused with the first butterfly level (pairs k, k + R/2):
+        //   p = x_k w_k,  r = p + x_{k+R/2} w_{k+R/2} (four FMAs),  d = 2 p - r
+        constexpr int NI = NP / R, H = R / 2;
         const C *tws = tw + Sched<N>::twoff(I) + (u % Mi);
 #pragma unroll
         for (int s = 0; s < S; ++s) {
 #pragma unroll
-            for (int k = 1; k < R; ++k) {
-                const C w = tws[(k - 1) * NI + s * Mi];
-                x[k * S + s] = SIGN < 0 ? cmul(x[k * S + s], w) : cmulc(x[k * S + s], w);
+            for (int k = 0; k < H; ++k) {
+                C p = x[k * S + s];
+                if (k > 0) {
+                    const C w = tws[(k - 1) * NI + s * Mi];
+                    p = SIGN < 0 ? cmul(p, w) : cmulc(p, w);
+                }
+                const C b = x[(k + H) * S + s];
+                C w2 = tws[(k + H - 1) * NI + s * Mi];
+                if (SIGN > 0) w2.y = -w2.y;  // conjugate
+                C r;
+                r.x = fma(-w2.y, b.y, fma(w2.x, b.x, p.x));
+                r.y = fma(w2.y, b.x, fma(w2.x, b.y, p.y));
+                x[(k + H) * S + s] = mk<C>(fma((T)2, p.x, -r.x), fma((T)2, p.y, -r.y));
+                x[k * S + s] = r;
             }
         }
-    }
 #pragma unroll
-    for (int s = 0; s < S; ++s) dft_reg<R, S, SIGN>(&x[s]);
+        for (int s = 0; s < S; ++s) dft_reg<R, S, SIGN, C, false>(&x[s]);
+    } else {
+#pragma unroll
+        for (int s = 0; s < S; ++s) dft_reg<R, S, SIGN>(&x[s]);
+    }
 }
 
 // barrier over one group of a CTA (groups are independent pipelines that share only the twiddle table):

@@ -9,6 +9,8 @@
 //   MODE_OPEN   V/2 (natural order)  ->  forward DIF  ->  natural frequency order
 //   MODE_MID    inverse DIF  ->  merged potential phase V (permuted order)  ->  forward DIT
 //   MODE_CLOSE  inverse DIF  ->  natural order  ->  V/2
+//   MODE_CLOSE_OBS  the same, and the observables of the result (norm, autocorrelation with a reference state, <r>,
+//               one term of the eigenfunction filter) accumulated before it is stored
 //
 // (eq. 7, 98 eq. 11; the FFT stages are those of sso_pass.cuh).  As soon as the last exchange of a
 // tile has been read, the group's leader claims the next tile of the CTA, refills the buffer and asks L2 for
@@ -164,6 +166,7 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     constexpr int TWN = Sched<N>::twoff(LAST);
     constexpr int TWP = (TWN + 7) & ~7;
     constexpr bool EARLY = MODE == MODE_MID && (sizeof(T) == 4 || MAXT == 384);
+    constexpr bool OBS = MODE == MODE_CLOSE_OBS;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     C *stw = reinterpret_cast<C *>(smem_raw);
     C *bufs = stw + TWP;
@@ -228,6 +231,18 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
         ring.draw(grp);
     }
     gsync(gb);  // publishes the group's first ticket
+
+    // MODE_CLOSE_OBS: per-thread sums over all the tiles this thread meets
+    [[maybe_unused]] double ob[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    [[maybe_unused]] double fwr = 0.0, fwi = 0.0;
+    if constexpr (OBS) {
+        if (a.facc) {
+            sincos(a.fw_E * a.fw_t, &fwi, &fwr);
+            const double wdw = (1.0 - cospi(2.0 * a.fw_t / a.fw_T)) * a.fw_dts;
+            fwr *= wdw;
+            fwi *= wdw;
+        }
+    }
 
     for (;;) {
         const int k = ring.drawn(grp);  // the group's next tile, in the CTA's loading order
@@ -321,7 +336,42 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
             gsync(gb);
 #pragma unroll
             for (int q = 0; q < 16; ++q) x[q] = rb[lin_delta(q, U)];
-            if constexpr (MODE == MODE_CLOSE) phase(x);
+            if constexpr (MODE == MODE_CLOSE || OBS) phase(x);
+        }
+
+        if constexpr (OBS) {
+            // x is psi(t) in natural order: register q <-> position u + q U of line lic of component tile mod ncomp
+            const size_t e1 = (size_t)e0_ + (size_t)t * N + u;
+            double dsum = 0.0, dline = 0.0;
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                const double d = (double)x[q].x * (double)x[q].x + (double)x[q].y * (double)x[q].y;
+                dsum += d;
+                dline += d * (double)(u + q * U - a.obs_half[2]);
+            }
+            ob[0] += dsum;
+            if (a.obs_axL >= 0) ob[3 + a.obs_axL] += dline * a.obs_dx[2];
+            if (a.obs_axA >= 0) ob[3 + a.obs_axA] += dsum * (double)((lic >> a.rest1_shift) - a.obs_half[0]) * a.obs_dx[0];
+            if (a.obs_axB >= 0) ob[3 + a.obs_axB] += dsum * (double)((lic & (a.rest1 - 1)) - a.obs_half[1]) * a.obs_dx[1];
+            if (a.ref) {
+                const C *gr = reinterpret_cast<const C *>(a.ref) + e1;
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    const C r = ld_stream(gr + q * U);
+                    ob[1] += (double)r.x * (double)x[q].x + (double)r.y * (double)x[q].y;
+                    ob[2] += (double)r.x * (double)x[q].y - (double)r.y * (double)x[q].x;
+                }
+            }
+            if (a.facc) {
+                double2 *ga = reinterpret_cast<double2 *>(a.facc) + e1;
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    double2 v = ga[q * U];
+                    v.x += fwr * (double)x[q].x - fwi * (double)x[q].y;
+                    v.y += fwr * (double)x[q].y + fwi * (double)x[q].x;
+                    ga[q * U] = v;
+                }
+            }
         }
 
         // the buffer was written with ordinary (generic-proxy) stores and is refilled by the bulk-copy engine (async
@@ -337,6 +387,22 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
 #pragma unroll
             for (int q = 0; q < 16; ++q) st_stream(gout + q * U, x[q]);
         }
+    }
+    if constexpr (OBS) {
+        // warp sums by shuffles, CTA sums by shared-memory atomics, one row of partial sums per CTA (a final kernel adds
+        // the rows in a fixed order; which tiles a warp met depends on the tile pool, so the last bits may differ from run to run)
+        double *cta = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(bufs + (size_t)a.NB * a.bufstride) + 448);
+        __syncthreads();  // every group has left the tile loop
+        if (threadIdx.x < 6) cta[threadIdx.x] = 0.0;
+        __syncthreads();
+#pragma unroll
+        for (int v = 0; v < 6; ++v) {
+            double s = ob[v];
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+            if ((threadIdx.x & 31) == 0) atomicAdd(&cta[v], s);
+        }
+        __syncthreads();
+        if (threadIdx.x < 6) a.obs_partial[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = cta[threadIdx.x];
     }
 }
 

@@ -148,3 +148,59 @@ def test_observable_argument_errors(torch):
     assert L.sso_filter_accumulate(p._h, None, None, 0.0, 1.0, 0.0, 0.1, None) == sso.ERR_INVALID
     assert L.sso_overlap(None, None, None, out, None) == sso.ERR_INVALID
     p.destroy()
+
+
+FUSED = [
+    ("2d-c128-field", 1, (64, 128), (0.2, 0.1), sso.C128, True),
+    ("3d-dirac4-c128", 4, (16, 32, 64), (0.3, 0.2, 0.1), sso.C128, False),
+    ("2d-dirac2-c64", 2, (32, 256), (0.25, 0.1), sso.C64, False),
+    ("3d-c128", 1, (32, 16, 64), (0.3, 0.3, 0.2), sso.C128, False),
+    ("1d-c128", 1, (1024,), (0.1,), sso.C128, False),
+]
+
+
+@pytest.mark.parametrize("name,ncomp,sizes,dx,prec,field", FUSED, ids=[c[0] for c in FUSED])
+def test_observables_fused_into_the_closing_pass(torch, name, ncomp, sizes, dx, prec, field):
+    """sso_step_observe: norm, <ref|psi>, <r> and one filter term come out of the closing pass of the call; they equal
+    the oracle's observables of the oracle's psi after the same steps, and psi itself equals plain sso_step."""
+    rng = np.random.default_rng(5000 + [c[0] for c in FUSED].index(name))
+    cdt = np.complex128 if prec == sso.C128 else np.complex64
+    tau = 0.01 if ncomp == 1 else 1e-4
+    psi0 = packet(rng, ncomp, sizes, dx).astype(cdt)
+    ref = packet(rng, ncomp, sizes, dx).astype(cdt)
+    V = rng.uniform(-1.0, 1.0, size=sizes)
+    nsteps = 7
+    p = sso.Plan(sizes, dx, tau, ncomp, prec)
+    o = oracle.Solver(sizes, dx, tau, ncomp)
+    p.set_potential(V)
+    o.set_potential(V)
+    if field:
+        avg = rng.uniform(-0.3, 0.3, size=(nsteps, len(sizes)))
+        p.set_field(sso.FIELD_E, np.ascontiguousarray(avg))
+        o.set_field(oracle.FIELD_E, avg)
+    want = o.step(psi0.astype(np.complex128), nsteps)
+    acc0 = (rng.normal(size=(ncomp,) + tuple(sizes)) + 1j * rng.normal(size=(ncomp,) + tuple(sizes)))
+    want_acc = acc0.copy()
+    ft, fT, fE, fdts = 0.35, 1.3, -0.42, 0.05
+    o.filter_accumulate(want_acc, want, ft, fT, fE, fdts)
+    psi = torch.from_numpy(psi0).cuda()
+    tref = torch.from_numpy(ref).cuda()
+    acc = torch.from_numpy(acc0).cuda()
+    nrm, chi, r = p.step_observe(psi, nsteps, tref, acc, ft, fT, fE, fdts)
+    torch.cuda.synchronize()
+    tol = 1e-11 if prec == sso.C128 else 2e-5
+    got = psi.cpu().numpy()
+    assert np.linalg.norm((got - want).ravel()) / np.linalg.norm(want.ravel()) < tol
+    assert abs(nrm - o.norm(want)) < tol * 10
+    assert abs(chi - o.overlap(ref.astype(np.complex128), want)) < tol * 10
+    np.testing.assert_allclose(r, o.expect_r(want), atol=tol * 100)
+    assert np.abs(acc.cpu().numpy() - want_acc).max() < tol * 10 * np.abs(want_acc).max()
+    # the same psi as plain stepping, and the same numbers as the separate kernels on it
+    psi2 = torch.from_numpy(psi0).cuda()
+    p.set_time_index(0)
+    p.step(psi2, nsteps)
+    assert np.array_equal(psi2.cpu().numpy(), got)
+    assert abs(p.norm(psi2) - nrm) < 1e-13
+    assert abs(p.overlap(tref, psi2) - chi) < 1e-13
+    np.testing.assert_allclose(p.expect_position(psi2), r, atol=1e-12)
+    p.destroy()
