@@ -87,7 +87,7 @@ extern "C" {
 #define SSO_OPT_THREADS_PER_CTA 6        /* ring pipeline CTA size: 512 (128 regs/thread) or 384 (168); 0 = auto */
 
 #define SSO_MIN_AXIS 16   /* smallest supported axis length                       */
-#define SSO_MAX_AXIS 4096 /* largest supported axis length (one CTA holds a line) */
+#define SSO_MAX_AXIS 8192 /* largest supported axis length: one CTA of 512 threads holds a line (16 points per thread) */
 #define SSO_MAX_AXIS_1D 32768 /* 1D Schroedinger lattices (ncomp = 1, no SSO_FIELD_E, no position-space A): the line is
                                  spread over a thread-block cluster of 8 SMs                                         */
 

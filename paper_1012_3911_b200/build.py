@@ -22,7 +22,7 @@ HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 OBJ = HERE / "build"
 LIB = HERE / "libsso.so"
-ALL_SIZES = [16, 32, 64, 128, 256, 512, 1024, 2048, 4096]
+ALL_SIZES = [16, 32, 64, 128, 256, 512, 1024, 2048, 4096, 8192]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=default",

@@ -26,6 +26,8 @@
 #include "sso_line1d_args.h"
 
 // cluster size the 4096-point 1D line uses by default (0: the single-CTA kernel); chosen by measurement on B200
+// points of a 1D line one CTA's registers hold (sso_line1d.cuh); longer Schroedinger lines go to a cluster
+#define SSO_MAX_LINE_CTA 4096
 #ifndef SSO_CLUSTER_AUTO_4096
 #define SSO_CLUSTER_AUTO_4096 8
 #endif
@@ -421,6 +423,14 @@ static int freq_of_pos(int N, int p) {
     return f;
 }
 
+// bytes of shared memory the kernels give the twiddle blocks of an n-point line: none for the longest lines, whose
+// kernels read them from global memory (sso_pass.cuh, twiddles_in_global)
+static int twiddle_count_padded(int N);
+static size_t twiddle_smem_bytes(int n, size_t esz) {
+    const size_t tw = (size_t)twiddle_count_padded(n) * esz;
+    return (tw + (size_t)(n + n / 16) * esz > (size_t)200 * 1024) ? 0 : tw;
+}
+
 // entries of the twiddle blocks of all non-final stages, padded as in the kernel (TWP)
 static int twiddle_count_padded(int N) {
     HostSched s(N);
@@ -641,7 +651,7 @@ int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double
         // a 1D Schroedinger line may be spread over a thread-block cluster (sso_line1d_cluster.cuh)
         const int64_t nmax = (ndim == 1 && ncomp == 1) ? SSO_MAX_AXIS_1D : SSO_MAX_AXIS;
         if (sizes[a] < SSO_MIN_AXIS || sizes[a] > nmax)
-            return fail(nullptr, SSO_ERR_UNSUPPORTED, "axis length outside [16, 4096] (1D Schroedinger lattices: [16, 32768])");
+            return fail(nullptr, SSO_ERR_UNSUPPORTED, "axis length outside [16, 8192] (1D Schroedinger lattices: [16, 32768])");
     }
     if (ncomp > 1 && (long long)ncomp * (sizes[0] / 16) > 512)
         return fail(nullptr, SSO_ERR_UNSUPPORTED, "Dirac plans need ncomp * sizes[0] <= 8192 (all components of a line share one CTA)");
@@ -1122,7 +1132,7 @@ int launch(sso_plan *plan, void *psi, const PassSpec &s, cudaStream_t st) {
     const int GT = cc * TL * U;
     size_t greg = (size_t)cc * TL * pitch * esz + (size_t)TL * esz + 2 * sizeof(int);
     greg = (greg + 127) & ~(size_t)127;
-    const size_t twbytes = (size_t)twiddle_count_padded(A.n) * esz;
+    const size_t twbytes = twiddle_smem_bytes(A.n, (size_t)esz);
     int G = 1;
     if (GT % 32 == 0) {
         const int maxthreads = 512;
@@ -1191,7 +1201,7 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     const int pitch = A.n + A.n / 16;
     size_t bufbytes = (size_t)TL * pitch * esz;
     bufbytes = (bufbytes + 127) & ~(size_t)127;
-    const size_t twbytes = (size_t)twiddle_count_padded(A.n) * esz;
+    const size_t twbytes = twiddle_smem_bytes(A.n, (size_t)esz);
     const long long ntiles = lines * plan->ncomp / TL;
     if (ntiles > 0x7fffffffLL) return fail(plan, SSO_ERR_UNSUPPORTED, "too many tiles");
     // G groups, each with its own NBG buffers (NBG = 2: the next tile loads while the current one is worked on)
@@ -1530,10 +1540,10 @@ int build_ktab(sso_plan *plan, long long n, cudaStream_t st) {
 int cluster_size_for(const sso_plan *p) {
     if (p->ndim != 1 || p->ncomp != 1 || p->field_kind == SSO_FIELD_E || p->d_apos || p->opt_cluster == 1) return 0;
     const int n = p->ax[0].n;
-    auto usable = [&](int cs) { return n / cs >= 512 && n / cs <= SSO_MAX_AXIS && find_line1d_cluster(p->precision, n / cs, cs) != nullptr; };
+    auto usable = [&](int cs) { return n / cs >= 512 && n / cs <= SSO_MAX_LINE_CTA && find_line1d_cluster(p->precision, n / cs, cs) != nullptr; };
     if (p->opt_cluster > 1) return usable(p->opt_cluster) ? p->opt_cluster : 0;
-    if (n > SSO_MAX_AXIS) return usable(8) ? 8 : (usable(4) ? 4 : 0);
-    return (n == SSO_MAX_AXIS && usable(SSO_CLUSTER_AUTO_4096)) ? SSO_CLUSTER_AUTO_4096 : 0;
+    if (n > SSO_MAX_LINE_CTA) return usable(8) ? 8 : (usable(4) ? 4 : 0);
+    return (n == SSO_MAX_LINE_CTA && usable(SSO_CLUSTER_AUTO_4096)) ? SSO_CLUSTER_AUTO_4096 : 0;
 }
 
 int build_cluster_tables(sso_plan *plan, int cs) {
@@ -1662,7 +1672,7 @@ static int step_impl(sso_plan *plan, void *psi, int64_t nsteps, void *stream, Ob
         const long long chunk = (kshift || plan->d_apos) ? 1 : nsteps;
         const int cs = cluster_size_for(plan);
         if (!cs && plan->ax[0].n > SSO_MAX_AXIS)
-            return fail(plan, SSO_ERR_UNSUPPORTED, "1D lattices beyond 4096 points run on a thread-block cluster: Schroedinger without a length-gauge field only");
+            return fail(plan, SSO_ERR_UNSUPPORTED, "1D lattices beyond 8192 points run on a thread-block cluster: Schroedinger without a length-gauge field only");
         if (cs && (rc = build_cluster_tables(plan, cs)) != SSO_OK) return rc;
         for (long long s = 0; s < nsteps; s += chunk) {
             if (chunk > 0x7fffffffLL) return fail(plan, SSO_ERR_INVALID, "nsteps too large");

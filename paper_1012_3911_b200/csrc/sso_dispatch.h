@@ -60,7 +60,7 @@ struct PassArgs {
 using LaunchFn = cudaError_t (*)(const PassArgs &, unsigned threads, size_t smem, cudaStream_t st);
 
 // one lookup function per compiled (precision, line length); returns NULL for a variant that is not built
-#define SSO_FOR_EACH_N(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096)
+#define SSO_FOR_EACH_N(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096) X(8192)
 #define SSO_DECL_LOOKUP(N)                                         \
     LaunchFn sso_lookup_f32_##N(int strided, int pw, int sign);    \
     LaunchFn sso_lookup_f64_##N(int strided, int pw, int sign);

@@ -128,7 +128,10 @@ template <typename T, int M, int CS> cudaError_t launch_line1d_cluster(const Lin
 
 #define SSO_CAT4_(a, b, c) a##b##_##c
 #define SSO_CAT4(a, b, c) SSO_CAT4_(a, b, c)
-#ifdef SSO_STUB
+// lines beyond 4096 points (one 512-thread group, twiddles read from global memory for complex128) run on the
+// contiguous-axis ring and the direct kernel only: no strided tile of theirs fits a ring buffer, and the 1D
+// register-resident kernels hold at most 4096 points per CTA
+#if defined(SSO_STUB) || SSO_N > 4096
 SRingLaunchFn SSO_CAT4(sso_sring_lookup_, SSO_TNAME, SSO_N)(int) { return nullptr; }
 #else
 SRingLaunchFn SSO_CAT4(sso_sring_lookup_, SSO_TNAME, SSO_N)(int mode) {
@@ -145,13 +148,13 @@ SRingLaunchFn SSO_CAT4(sso_sring_lookup_, SSO_TNAME, SSO_N)(int mode) {
 }
 #endif
 
-#ifdef SSO_STUB
+#if defined(SSO_STUB) || SSO_N > 4096
 Line1dLaunchFn SSO_CAT4(sso_line1d_lookup_, SSO_TNAME, SSO_N)() { return nullptr; }
 #else
 Line1dLaunchFn SSO_CAT4(sso_line1d_lookup_, SSO_TNAME, SSO_N)() { return &launch_line1d<SSO_T, SSO_N>; }
 #endif
 
-#if defined(SSO_STUB) || SSO_N < 512
+#if defined(SSO_STUB) || SSO_N < 512 || SSO_N > 4096
 Line1dClusterLaunchFn SSO_CAT4(sso_line1d_cluster_lookup_, SSO_TNAME, SSO_N)(int) { return nullptr; }
 #else
 Line1dClusterLaunchFn SSO_CAT4(sso_line1d_cluster_lookup_, SSO_TNAME, SSO_N)(int cs) {
@@ -172,12 +175,15 @@ RingLaunchFn SSO_CAT4(sso_ring_lookup_, SSO_TNAME, SSO_N)(int mode, int maxt) {
         if (mode == MODE_MID) return &launch_ring<T, N, MODE_MID, +1, 512>;
         if (mode == MODE_CLOSE) return &launch_ring<T, N, MODE_CLOSE, +1, 512>;
         if (mode == MODE_CLOSE_OBS) return &launch_ring<T, N, MODE_CLOSE_OBS, +1, 512>;
-    } else if (maxt == 384) {
+    }
+#if SSO_N <= 4096
+    else if (maxt == 384) {
         if (mode == MODE_OPEN) return &launch_ring<T, N, MODE_OPEN, -1, 384>;
         if (mode == MODE_MID) return &launch_ring<T, N, MODE_MID, +1, 384>;
         if (mode == MODE_CLOSE) return &launch_ring<T, N, MODE_CLOSE, +1, 384>;
         if (mode == MODE_CLOSE_OBS) return &launch_ring<T, N, MODE_CLOSE_OBS, +1, 384>;
     }
+#endif
     return nullptr;
 }
 #endif

@@ -97,6 +97,12 @@ template <int N> struct Sched {
     }
 };
 
+// The twiddle blocks of a line sit in shared memory beside the line buffers -- except for the longest lines
+// (8192 complex128 points: 131 KB of twiddles + 139 KB of line), whose kernels read them from global memory (L2)
+template <typename C, int N> __host__ __device__ constexpr bool twiddles_in_global() {
+    return (size_t)(((Sched<N>::twoff(Sched<N>::M - 1) + 7) & ~7) + N + N / 16) * sizeof(C) > (size_t)200 * 1024;
+}
+
 // cos(2 pi j/16), sin(2 pi j/16), j = 0..7
 __host__ __device__ constexpr double cos16(int j) {
     return j == 0 ? 1.0
@@ -463,9 +469,10 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
     constexpr int LAST = Sched<N>::M - 1;
     constexpr int TWN = Sched<N>::twoff(LAST);
     constexpr int TWP = (TWN + 7) & ~7;  // keep the exchange buffer 128-byte aligned
+    constexpr bool TWG = twiddles_in_global<C, N>();
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    C *stw = reinterpret_cast<C *>(smem_raw);
-    C *sm = stw + TWP;
+    const C *stw = TWG ? reinterpret_cast<const C *>(a.tw) : reinterpret_cast<const C *>(smem_raw);
+    C *sm = reinterpret_cast<C *>(smem_raw) + (TWG ? 0 : TWP);
 
     const int TL = a.TL;
     // groups: G independent pipelines of GT = CC * TL * U threads each; a group owns an exchange buffer,
@@ -492,9 +499,10 @@ __global__ void __launch_bounds__(512, (sizeof(T) == 4 ? 2 : 1)) pass_kernel(con
     int *snext = reinterpret_cast<int *>(lsc + TL);         // tile scheduler mailbox [2]
 
     // twiddles -> shared memory, once per CTA
-    {
+    if constexpr (!TWG) {
         const C *__restrict__ gtw = reinterpret_cast<const C *>(a.tw);
-        for (int i = threadIdx.x; i < TWN; i += blockDim.x) stw[i] = gtw[i];
+        C *dst = reinterpret_cast<C *>(smem_raw);
+        for (int i = threadIdx.x; i < TWN; i += blockDim.x) dst[i] = gtw[i];
     }
     if (tid == 0) snext[0] = (int)atomicAdd(&a.sched[0], 1u);
     __syncthreads();

@@ -167,9 +167,10 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     constexpr int TWP = (TWN + 7) & ~7;
     constexpr bool EARLY = MODE == MODE_MID && (sizeof(T) == 4 || MAXT == 384);
     constexpr bool OBS = MODE == MODE_CLOSE_OBS;
+    constexpr bool TWG = twiddles_in_global<C, N>();  // the longest lines read their twiddles from global memory
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    C *stw = reinterpret_cast<C *>(smem_raw);
-    C *bufs = stw + TWP;
+    const C *stw = TWG ? reinterpret_cast<const C *>(a.tw) : reinterpret_cast<const C *>(smem_raw);
+    C *bufs = reinterpret_cast<C *>(smem_raw) + (TWG ? 0 : TWP);
     TileRing ring(bufs + (size_t)a.NB * a.bufstride, a.NB, a.G);
 
     const int TL = a.TL, GT = a.GT, G = a.G, NB = a.NB;
@@ -212,9 +213,10 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
     // let the next pass of the stream start its own setup as SMs free up
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     ring.init();
-    {
+    if constexpr (!TWG) {
         const C *__restrict__ gtw = reinterpret_cast<const C *>(a.tw);
-        for (int i = threadIdx.x; i < TWN; i += blockDim.x) stw[i] = gtw[i];
+        C *dst = reinterpret_cast<C *>(smem_raw);
+        for (int i = threadIdx.x; i < TWN; i += blockDim.x) dst[i] = gtw[i];
     }
     __syncthreads();
     // everything above touched only plan-owned tables; psi is valid once the previous pass has completed

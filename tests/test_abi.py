@@ -49,7 +49,7 @@ def _create(L, ndim, sizes, dx, dt, ncomp, prec):
         ((1, (8,), (0.1,), 0.01, 1, sso.C128), sso.ERR_UNSUPPORTED),       # below SSO_MIN_AXIS
         ((1, (65536,), (0.1,), 0.01, 1, sso.C128), sso.ERR_UNSUPPORTED),   # above SSO_MAX_AXIS_1D
         ((1, (8192,), (0.1,), 0.01, 2, sso.C128), sso.ERR_UNSUPPORTED),    # above SSO_MAX_AXIS for a 1D Dirac spinor
-        ((2, (8192, 64), (0.1, 0.1), 0.01, 1, sso.C128), sso.ERR_UNSUPPORTED),  # above SSO_MAX_AXIS for a 2D lattice
+        ((2, (16384, 64), (0.1, 0.1), 0.01, 1, sso.C128), sso.ERR_UNSUPPORTED),  # above SSO_MAX_AXIS for a 2D lattice
         ((2, (64, 64), (0.1, -0.1), 0.01, 1, sso.C128), sso.ERR_INVALID),  # dx <= 0
         ((2, (64, 64), (0.1, float("nan")), 0.01, 1, sso.C128), sso.ERR_INVALID),
         ((1, (64,), (0.1,), float("inf"), 1, sso.C128), sso.ERR_INVALID),  # dt not finite

@@ -91,11 +91,11 @@ def test_cluster_line_random_state_and_vector_potential(torch):
 
 
 def test_long_line_needs_the_cluster_path(torch):
-    w = wl.config1(sizes=(8192,), nsteps=4)
+    w = wl.config1(sizes=(16384,), nsteps=4)
     p = sso.Plan(w.sizes, w.dx, w.dt, 1, sso.C128)
     p.set_potential(w.V)
     psi = torch.from_numpy(w.psi0.astype(np.complex128)).cuda()
-    p.set_option(sso.OPT_CLUSTER_1D, 1)  # off: no single CTA holds 8192 points
+    p.set_option(sso.OPT_CLUSTER_1D, 1)  # off: no single CTA holds 16384 points
     with pytest.raises(sso.SsoError) as e:
         p.step(psi, 1)
     assert e.value.code == sso.ERR_UNSUPPORTED
@@ -105,3 +105,17 @@ def test_long_line_needs_the_cluster_path(torch):
         p.step(psi, 1)
     assert e.value.code == sso.ERR_UNSUPPORTED
     p.destroy()
+
+
+def test_8192_point_line_on_one_cta(torch):
+    """8192 points are the most one CTA holds (512 threads x 16 points, twiddles read from global memory for
+    complex128): with the cluster switched off, or with a length-gauge field, the direct kernel takes the line."""
+    w = wl.config1(sizes=(8192,), nsteps=20)
+    got, nrm, psi0 = run_gpu(torch, w, 20, sso.C128, 1)
+    want = run_oracle(w, 20, psi0)
+    assert rel_l2(got, want) <= 1e-12
+    rng = np.random.default_rng(81)
+    avg = rng.uniform(-0.2, 0.2, size=(6, 1))
+    got, nrm, psi0 = run_gpu(torch, w, 6, sso.C64, 0, field=(sso.FIELD_E, np.ascontiguousarray(avg)))
+    want = run_oracle(w, 6, psi0, field=(oracle.FIELD_E, avg))
+    assert rel_l2(got, want) <= 2e-5

@@ -299,3 +299,27 @@ def test_many_tiles_per_group_large_lattice(torch):
     assert err < 1e-13, err
     p.destroy()
     p2.destroy()
+
+
+LONG_AXIS = [
+    ("2d-8192x32-c128", (8192, 32), sso.C128), ("2d-32x8192-c128", (32, 8192), sso.C128),
+    ("2d-8192x64-c64", (8192, 64), sso.C64), ("2d-16x8192-c64", (16, 8192), sso.C64),
+    ("3d-16x8192x16-c128", (16, 8192, 16), sso.C128),
+]
+
+
+@pytest.mark.parametrize("name,sizes,prec", LONG_AXIS, ids=[c[0] for c in LONG_AXIS])
+def test_axis_of_8192_points(torch, name, sizes, prec):
+    """SSO_MAX_AXIS = 8192: the longest line one CTA holds (512 threads x 16 points; the complex128 kernels read its
+    twiddles from global memory).  Schroedinger with a field on the long axis, unstructured noise, 6 steps."""
+    nd = len(sizes)
+    rng = np.random.default_rng(8192 + nd + sizes[0])
+    w = wl.config2(sizes=sizes[:2], nsteps=6) if nd == 2 else wl.config3(sizes=sizes, nsteps=6)
+    psi0 = wl.random_state(sizes, 1, 8192, w.dx)
+    avg = np.zeros((6, nd))
+    avg[:, int(np.argmax(sizes))] = rng.uniform(-0.05, 0.05, size=6)
+    w.field_kind, w.step_avg = sso.FIELD_E, avg
+    got, nrm = gpu_steps(torch, w, 6, prec, psi0=psi0.astype(np.complex128 if prec == sso.C128 else np.complex64))
+    want = oracle_steps(w, 6, prec, psi0=psi0.astype(np.complex128 if prec == sso.C128 else np.complex64))
+    assert rel_l2(got, want) <= TOL[prec] * 0.1
+    assert abs(nrm - 1.0) < (1e-11 if prec == sso.C128 else 1e-4)
