@@ -189,6 +189,51 @@ __global__ void apos_rotate_kernel(void *__restrict__ psi_, const double *__rest
     }
 }
 
+// Dirac kinetic factor as a kernel of its own, for lines whose components do not fit one CTA together (ncomp * n_0 >
+// 8192): psi is in momentum space on every axis (axis 0 in network order, as the transform-only passes leave it), one
+// thread per k point holds all components and applies U = cos(E tau) - i (sin(E tau)/E) (c alpha.pi + m c^2 beta)
+// (eq. 27-33 in the closed form of sso_sring.cuh; pi = k - q Abar_n, reading G16), times 1/Ntot.
+template <typename T, int CC>
+__global__ void dirac_pointwise_kernel(void *__restrict__ psi_, long long npts, long long inner, int rest1, const double *__restrict__ k0pos,
+                                       const double *__restrict__ kv1, const double *__restrict__ kv2, double sh0, double sh1, double sh2,
+                                       double mass, double clight, double dt, double scale) {
+    using C = typename Cx2<T>::type;
+    C *psi = reinterpret_cast<C *>(psi_);
+    const double mc2 = mass * clight * clight;
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < npts; j += (long long)gridDim.x * blockDim.x) {
+        const long long i0 = j / inner, line = j % inner;
+        const double p0 = k0pos[i0] - sh0;
+        const double p1 = kv1 ? kv1[line / rest1] - sh1 : (kv2 ? kv2[line % rest1] - sh1 : 0.0);
+        const double p2 = kv1 ? kv2[line % rest1] - sh2 : 0.0;
+        const double E = sqrt(clight * clight * (p0 * p0 + p1 * p1 + p2 * p2) + mc2 * mc2);
+        double sn, cs;
+        sincos(E * dt, &sn, &cs);
+        const double sE = (E > 0.0 ? sn / E : dt) * scale;
+        cs *= scale;
+        const T fc = (T)cs, fm = (T)(sE * mc2), f0 = (T)(sE * clight * p0), f1 = (T)(sE * clight * p1), f2 = (T)(sE * clight * p2);
+        // out = cs psi - i sE H psi ;  (-i)(a + i b) = b - i a
+        if (CC == 2) {
+            const C a0 = psi[j], a1 = psi[npts + j];
+            // H psi_0 = mc2 a0 + c (p0 - i p1) a1 ; H psi_1 = c (p0 + i p1) a0 - mc2 a1
+            const T h0x = fm * a0.x + f0 * a1.x + f1 * a1.y, h0y = fm * a0.y + f0 * a1.y - f1 * a1.x;
+            const T h1x = f0 * a0.x - f1 * a0.y - fm * a1.x, h1y = f0 * a0.y + f1 * a0.x - fm * a1.y;
+            psi[j] = C{fc * a0.x + h0y, fc * a0.y - h0x};
+            psi[npts + j] = C{fc * a1.x + h1y, fc * a1.y - h1x};
+        } else {
+            const C a0 = psi[j], a1 = psi[npts + j], a2 = psi[2 * npts + j], a3 = psi[3 * npts + j];
+            // sigma.p (v0, v1) = (p2 v0 + (p0 - i p1) v1, (p0 + i p1) v0 - p2 v1);  H psi = (mc2 u + c sigma.p l, c sigma.p u - mc2 l)
+            const T h0x = fm * a0.x + f2 * a2.x + f0 * a3.x + f1 * a3.y, h0y = fm * a0.y + f2 * a2.y + f0 * a3.y - f1 * a3.x;
+            const T h1x = fm * a1.x + f0 * a2.x - f1 * a2.y - f2 * a3.x, h1y = fm * a1.y + f0 * a2.y + f1 * a2.x - f2 * a3.y;
+            const T h2x = f2 * a0.x + f0 * a1.x + f1 * a1.y - fm * a2.x, h2y = f2 * a0.y + f0 * a1.y - f1 * a1.x - fm * a2.y;
+            const T h3x = f0 * a0.x - f1 * a0.y - f2 * a1.x - fm * a3.x, h3y = f0 * a0.y + f1 * a0.x - f2 * a1.y - fm * a3.y;
+            psi[j] = C{fc * a0.x + h0y, fc * a0.y - h0x};
+            psi[npts + j] = C{fc * a1.x + h1y, fc * a1.y - h1x};
+            psi[2 * npts + j] = C{fc * a2.x + h2y, fc * a2.y - h2x};
+            psi[3 * npts + j] = C{fc * a3.x + h3y, fc * a3.y - h3x};
+        }
+    }
+}
+
 // norm: partial sums of |psi|^2 in double, warp-shuffle tree, fixed order (deterministic)
 template <typename T>
 __global__ void norm_partial_kernel(const void *__restrict__ psi, long long count, double *__restrict__ partial) {
@@ -653,8 +698,8 @@ int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double
         if (sizes[a] < SSO_MIN_AXIS || sizes[a] > nmax)
             return fail(nullptr, SSO_ERR_UNSUPPORTED, "axis length outside [16, 8192] (1D Schroedinger lattices: [16, 32768])");
     }
-    if (ncomp > 1 && (long long)ncomp * (sizes[0] / 16) > 512)
-        return fail(nullptr, SSO_ERR_UNSUPPORTED, "Dirac plans need ncomp * sizes[0] <= 8192 (all components of a line share one CTA)");
+    if (ndim == 1 && ncomp > 1 && (long long)ncomp * (sizes[0] / 16) > 512)
+        return fail(nullptr, SSO_ERR_UNSUPPORTED, "1D Dirac plans need ncomp * sizes[0] <= 8192 (all components of the line share one CTA)");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         cudaGetLastError();
@@ -1358,7 +1403,7 @@ SRingShape sring_shape(const sso_plan *plan, int axis, int cc, bool light) {
 }
 
 int launch_sring_pass(sso_plan *plan, void *psi, int axis, int smode, long long n, const SRingShape &sh, cudaStream_t st) {
-    PassTimer timer(plan, smode == SMODE_DIF ? SSO_PASS_MIDDLE_FORWARD : (smode == SMODE_DIT ? SSO_PASS_MIDDLE_INVERSE : SSO_PASS_KINETIC), st);
+    PassTimer timer(plan, axis == 0 ? SSO_PASS_KINETIC : (smode == SMODE_DIF ? SSO_PASS_MIDDLE_FORWARD : SSO_PASS_MIDDLE_INVERSE), st);
     const Axis &A = plan->ax[axis];
     const Geometry g = geometry(plan, axis);
     const int esz = (int)plan->esize();
@@ -1611,6 +1656,33 @@ int build_kphase_cluster(sso_plan *plan, long long n, cudaStream_t st) {
     return SSO_OK;
 }
 
+// Dirac lines whose components do not fit one CTA together: the kinetic sandwich is split into a transform-only pass
+// per direction and the pointwise kernel (two more round trips of psi per step)
+bool dirac_split_kinetic(const sso_plan *p) { return p->ncomp > 1 && p->ndim >= 2 && (long long)p->ncomp * (p->ax[0].n / 16) > 512; }
+
+int launch_dirac_pointwise(sso_plan *plan, void *psi, long long n, cudaStream_t st) {
+    PassTimer timer(plan, SSO_PASS_KINETIC, st);
+    const Geometry g = geometry(plan, 0);
+    double sh[3] = {0.0, 0.0, 0.0};
+    if (plan->field_kind == SSO_FIELD_A)
+        for (int ax = 0; ax < plan->ndim; ++ax) sh[ax] = plan->charge * plan->h_avg[(size_t)n * plan->ndim + ax];
+    const double *kv1 = g.oaxA >= 0 ? plan->ax[g.oaxA].d_kv : nullptr, *kv2 = g.oaxB >= 0 ? plan->ax[g.oaxB].d_kv : nullptr;
+    const int blocks = plan->num_sms * 8;
+    const double scale = 1.0 / (double)plan->npts;
+#define SSO_DPW(TT, CCN)                                                                                                                      \
+    dirac_pointwise_kernel<TT, CCN><<<blocks, 256, 0, st>>>(psi, plan->npts, g.inner, g.rest1, plan->ax[0].d_kpos, kv1, kv2, sh[0], sh[1], sh[2], \
+                                                            plan->mass, plan->clight, plan->dt, scale)
+    if (plan->precision == SSO_C128) {
+        if (plan->ncomp == 2) SSO_DPW(double, 2);
+        else SSO_DPW(double, 4);
+    } else {
+        if (plan->ncomp == 2) SSO_DPW(float, 2);
+        else SSO_DPW(float, 4);
+    }
+#undef SSO_DPW
+    return pass_status(plan, "Dirac pointwise kinetic kernel", cudaGetLastError());
+}
+
 int kinetic_pw(const sso_plan *p) { return p->ncomp == 1 ? PW_KS : (p->ncomp == 2 ? PW_KD2 : PW_KD4); }
 
 long long launches_for(const sso_plan *p, long long nsteps) {
@@ -1626,11 +1698,12 @@ long long launches_for(const sso_plan *p, long long nsteps) {
     }
     const long long chunk = p->d_apos ? 1 : erow_chunk(p);
     const long long nchunks = (nsteps + chunk - 1) / chunk;
-    if (p->ncomp > 1 && p->opt_dirac_table && sring_shape(p, 0, p->ncomp, false).ok) cnt += dirac_table_per_step(p) ? nsteps : (p->ktab_valid ? 0 : 1);  // Dirac kinetic table
+    if (p->ncomp > 1 && p->opt_dirac_table && !dirac_split_kinetic(p) && sring_shape(p, 0, p->ncomp, false).ok) cnt += dirac_table_per_step(p) ? nsteps : (p->ktab_valid ? 0 : 1);  // Dirac kinetic table
     bool eph = false;
     for (int a = 0; a < p->ndim; ++a) eph = eph || (p->field_kind == SSO_FIELD_E && p->e_axis_on[a]);
     cnt += nchunks * (eph ? 2 : 1);              // opening pass (+ field phase rows)
     cnt += nsteps * (p->ndim == 3 ? 3 : 1);      // kinetic sandwich (+ middle-axis DIF and DIT)
+    if (dirac_split_kinetic(p)) cnt += 2 * nsteps;  // transform, pointwise factor, transform instead of one sandwich
     cnt += nsteps;                               // potential sandwiches and the closing pass
     if (p->d_apos) cnt += 2 * nchunks;           // position-space rotations before every opening and after every closing pass
     if (kshift) cnt += nsteps * p->ndim;
@@ -1724,6 +1797,7 @@ static int step_impl(sso_plan *plan, void *psi, int64_t nsteps, void *stream, Ob
         const long long chunk = plan->d_apos ? 1 : erow_chunk(plan);
         SRingShape shk = sring_shape(plan, 0, plan->ncomp == 1 ? 1 : plan->ncomp, false);
         SRingShape shm = nd == 3 ? sring_shape(plan, 1, 1, true) : SRingShape{};
+        SRingShape sh0 = dirac_split_kinetic(plan) ? sring_shape(plan, 0, 1, true) : SRingShape{};
         for (long long c0 = 0; c0 < nsteps; c0 += chunk) {
             const long long ns = nsteps - c0 < chunk ? nsteps - c0 : chunk;
             const long long nb = n0 + c0;
@@ -1742,13 +1816,26 @@ static int step_impl(sso_plan *plan, void *psi, int64_t nsteps, void *stream, Ob
                     }
                     if (rc != SSO_OK) return rc;
                 }
-                if (shk.ok && (rc = build_ktab(plan, n, st)) != SSO_OK) return rc;
-                if (shk.ok) rc = launch_sring_pass(plan, psi, 0, kpw == PW_KS ? SMODE_KS : (kpw == PW_KD2 ? SMODE_KD2 : SMODE_KD4), n, shk, st);
-                else {
-                    PassSpec kin{0, kpw, -1, 1, 1, 0, 1, 0, 0, 1, n};  // F_0 K F_0^-1
-                    rc = launch(plan, psi, kin, st);
+                if (dirac_split_kinetic(plan)) {
+                    // F_0 (components one by one), the Dirac factor as a kernel of its own, F_0^-1
+                    for (int dir = 0; dir < 2; ++dir) {
+                        if (sh0.ok) rc = launch_sring_pass(plan, psi, 0, dir == 0 ? SMODE_DIF : SMODE_DIT, n, sh0, st);
+                        else {
+                            PassSpec tr{0, PW_NONE, -1, dir == 0, dir == 1, 0, 0, 0, 0, 1, n};
+                            rc = launch(plan, psi, tr, st);
+                        }
+                        if (rc != SSO_OK) return rc;
+                        if (dir == 0 && (rc = launch_dirac_pointwise(plan, psi, n, st)) != SSO_OK) return rc;
+                    }
+                } else {
+                    if (shk.ok && (rc = build_ktab(plan, n, st)) != SSO_OK) return rc;
+                    if (shk.ok) rc = launch_sring_pass(plan, psi, 0, kpw == PW_KS ? SMODE_KS : (kpw == PW_KD2 ? SMODE_KD2 : SMODE_KD4), n, shk, st);
+                    else {
+                        PassSpec kin{0, kpw, -1, 1, 1, 0, 1, 0, 0, 1, n};  // F_0 K F_0^-1
+                        rc = launch(plan, psi, kin, st);
+                    }
+                    if (rc != SSO_OK) return rc;
                 }
-                if (rc != SSO_OK) return rc;
                 if (nd == 3) {  // F_1^-1 from network order
                     if (shm.ok) rc = launch_sring_pass(plan, psi, 1, SMODE_DIT, n, shm, st);
                     else {

@@ -56,7 +56,7 @@ def _create(L, ndim, sizes, dx, dt, ncomp, prec):
         ((1, (64,), (0.1,), 0.01, 3, sso.C128), sso.ERR_INVALID),          # ncomp
         ((3, (16, 16, 16), (0.1,) * 3, 0.01, 2, sso.C128), sso.ERR_INVALID),  # 2 components in 3D
         ((1, (64,), (0.1,), 0.01, 1, 7), sso.ERR_INVALID),                 # precision
-        ((2, (4096, 64), (0.1, 0.1), 0.01, 4, sso.C128), sso.ERR_UNSUPPORTED),  # Dirac line too long for one CTA
+        ((1, (4096,), (0.1,), 0.01, 4, sso.C128), sso.ERR_UNSUPPORTED),    # 1D Dirac line too long for one CTA
     ],
 )
 def test_plan_create_rejects_bad_arguments(L, args, code):

@@ -323,3 +323,33 @@ def test_axis_of_8192_points(torch, name, sizes, prec):
     want = oracle_steps(w, 6, prec, psi0=psi0.astype(np.complex128 if prec == sso.C128 else np.complex64))
     assert rel_l2(got, want) <= TOL[prec] * 0.1
     assert abs(nrm - 1.0) < (1e-11 if prec == sso.C128 else 1e-4)
+
+
+LONG_DIRAC = [
+    ("2d-4096x16-4comp-c128", 4, (4096, 16), sso.C128, False), ("2d-8192x16-2comp-c128", 2, (8192, 16), sso.C128, True),
+    ("3d-4096x16x16-4comp-c64", 4, (4096, 16, 16), sso.C64, False), ("2d-2048x32-4comp-c128", 4, (2048, 32), sso.C128, True),
+]
+
+
+@pytest.mark.parametrize("name,ncomp,sizes,prec,field", LONG_DIRAC, ids=[c[0] for c in LONG_DIRAC])
+def test_dirac_lines_longer_than_one_cta_holds(torch, name, ncomp, sizes, prec, field):
+    """ncomp * n_0 > 8192: the components of a k point no longer meet in one CTA; the kinetic sandwich runs as
+    transform, pointwise Dirac kernel, transform.  (The last case, 4 x 2048, is the longest that still runs fused.)"""
+    nd = len(sizes)
+    rng = np.random.default_rng(4096 + ncomp + nd)
+    dx = (0.1,) * nd
+    grids = np.meshgrid(*[wl.axis_r(n, d) for n, d in zip(sizes, dx)], indexing="ij")
+    V = -1.0 / np.sqrt(sum(g * g for g in grids) + 1.0)
+    psi0 = wl.random_state(sizes, ncomp, 4096 + ncomp, dx)
+    nsteps = 5
+    w = wl.Workload(name, tuple(sizes), dx, 1e-4, ncomp, nsteps, psi0, V=V)
+    if field:
+        avg = np.zeros((nsteps, nd))
+        avg[:, 0] = rng.uniform(-5.0, 5.0, size=nsteps)
+        avg[:, nd - 1] = rng.uniform(-5.0, 5.0, size=nsteps)
+        w.field_kind, w.step_avg = sso.FIELD_A, avg
+    cdt = np.complex128 if prec == sso.C128 else np.complex64
+    got, nrm = gpu_steps(torch, w, nsteps, prec, psi0=psi0.astype(cdt))
+    want = oracle_steps(w, nsteps, prec, psi0=psi0.astype(cdt))
+    assert rel_l2(got, want) <= TOL[prec] * 0.1
+    assert abs(nrm - 1.0) < (1e-11 if prec == sso.C128 else 1e-4)
