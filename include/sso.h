@@ -97,7 +97,8 @@ typedef struct sso_plan sso_plan; /* opaque; owned by the library */
  * Create a plan for a lattice of `ndim` (1..3) axes with sizes[a] points (powers
  * of two in [SSO_MIN_AXIS, SSO_MAX_AXIS]; up to SSO_MAX_AXIS_1D for ndim = 1, ncomp = 1) and spacings dx[a] > 0, time step dt
  * (finite, may be negative: the Strang step is symmetric, so -dt undoes +dt),
- * ncomp = 1 (Schroedinger), 2 (Dirac, ndim 1 or 2) or 4 (Dirac, ndim 1..3).
+ * ncomp = 1 (Schroedinger), 2 (Dirac, ndim 1 or 2) or 4 (Dirac, ndim 1..3); a 1D Dirac plan needs
+ * ncomp * sizes[0] <= 8192 (SSO_ERR_UNSUPPORTED otherwise).
  * sizes and dx are host arrays, read during the call only.  Builds the radix
  * schedule, twiddle tables and k grids.  Defaults: V = 0, no
  * field, mass 1, c 137.036, charge -1 (electron), time index 0.

@@ -1255,7 +1255,8 @@ int launch_ring_pass(sso_plan *plan, void *psi, int mode, long long row, cudaStr
     if (bmax < 1) return fail(plan, SSO_ERR_UNSUPPORTED, "line too long for the ring pipeline");
     int G = 1, NB = 1;
     choose_groups(plan, GT, bmax, (ntiles + plan->num_sms - 1) / plan->num_sms, &G, &NB);
-    const int maxt = plan->opt_maxt ? plan->opt_maxt : (G * GT <= 384 ? 384 : 512);
+    // the 384-thread build (168 registers) only when the groups fit it; a knob that does not fit falls back
+    const int maxt = (plan->opt_maxt && G * GT <= plan->opt_maxt) ? plan->opt_maxt : (G * GT <= 384 && A.n <= 4096 ? 384 : 512);
     RingArgs a{};
     a.psi = psi;
     a.tw = A.tw;
