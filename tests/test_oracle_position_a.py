@@ -111,3 +111,27 @@ def test_position_space_factor_is_unitary_and_needs_a_spinor():
     s1.set_vector_potential(np.ones((1, 16)))
     with pytest.raises(ValueError):
         s1.step(np.ones((1, 16), complex), 1)
+
+
+def test_pulse_of_equation_46():
+    """workloads.pulse_*: eq. 46c envelope, E = omega dA/deta (eq. 46a with E = -dA/dt), A = 0 ahead
+    of the pulse, constant behind it, continuous everywhere."""
+    j, l, E0, omega = 8, 2, 3000.0, 2 * np.pi * 137.036 / 40.0
+    eta = np.linspace(-9 * np.pi, np.pi, 20001)
+    f = wl.pulse_envelope(eta, j, l)
+    assert f.max() == 1.0 and f.min() == 0.0
+    assert np.allclose(wl.pulse_envelope(np.array([-8 * np.pi, -7 * np.pi, -6 * np.pi, -4 * np.pi, -2 * np.pi, -np.pi, 0.0, 1.0, -30.0]), j, l),
+                       [0.0, 0.5, 1.0, 1.0, 1.0, 0.5, 0.0, 0.0, 0.0])
+    A = wl.pulse_vector_potential(eta, E0, omega, j, l)
+    dA = np.gradient(A, eta)
+    E = wl.pulse_field(eta, E0, j, l)
+    assert np.abs(omega * dA - E)[5:-5].max() < 2e-3 * E0  # second-order finite differences on a 5e-4 pi grid
+    assert np.all(A[eta >= 0] == 0.0)
+    behind = A[eta <= -j * np.pi]
+    assert np.ptp(behind) < 1e-9 * E0 / omega
+    # the step average tends to the midpoint value
+    x = np.linspace(-40.0, 0.0, 64)
+    k = omega / 137.036
+    avg = wl.pulse_step_average(x, 0.01, 1e-5, E0, omega, j, l, k)
+    mid = wl.pulse_vector_potential(k * x - omega * (0.01 + 0.5e-5), E0, omega, j, l)
+    assert np.abs(avg - mid).max() < 1e-6 * np.abs(mid).max()

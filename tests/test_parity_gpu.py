@@ -353,3 +353,34 @@ def test_dirac_lines_longer_than_one_cta_holds(torch, name, ncomp, sizes, prec, 
     want = oracle_steps(w, nsteps, prec, psi0=psi0.astype(cdt))
     assert rel_l2(got, want) <= TOL[prec] * 0.1
     assert abs(nrm - 1.0) < (1e-11 if prec == sso.C128 else 1e-4)
+
+
+def test_free_packet_in_the_laser_pulse_of_equation_46(torch):
+    """PAPER.md:400-412 (section V.3): a free 2D Dirac packet in a pulse travelling along x with E along y, the
+    vector potential A_y(k x - omega t) of eq. 46 applied in position space (eq. 26) and replaced every step by its
+    step average (sso_set_vector_potential); 2 and 4 components against the oracle."""
+    sizes, dx, tau, nsteps = (256, 64), (0.05, 0.05), 2e-5, 12
+    c, omega = wl.C_LIGHT, 2 * np.pi * wl.C_LIGHT / 8.0   # wavelength 8 a.u. so that the grid sees several half cycles
+    E0, j, l = 3000.0, 8, 2
+    X, Y = wl.mesh(sizes, dx)
+    for ncomp in (2, 4):
+        psi0 = wl.dirac_packet(sizes, dx, np.array([0.0, 0.0]), 2.0, ncomp, 1.0, c)
+        p = sso.Plan(sizes, dx, tau, ncomp, sso.C128)
+        o = oracle.Solver(sizes, dx, tau, ncomp)
+        psi = torch.from_numpy(psi0).cuda()
+        ref = psi0.copy()
+        for n in range(nsteps):
+            t = 4e-3 + n * tau  # the pulse front has reached the packet
+            A = np.zeros((2,) + sizes)
+            A[1] = wl.pulse_step_average(X, t, tau, E0, omega, j, l, omega / c)
+            assert np.abs(A[1]).max() > 1.0
+            p.set_vector_potential(np.ascontiguousarray(A))
+            o.set_vector_potential(A)
+            p.step(psi, 1)
+            ref = o.step(ref, 1)
+        torch.cuda.synchronize()
+        got = psi.cpu().numpy()
+        assert rel_l2(got, ref) <= 1e-12
+        assert abs(p.norm(psi) - 1.0) < 1e-12
+        assert rel_l2(got, psi0) > 1e-3  # the pulse did act on the packet
+        p.destroy()

@@ -230,6 +230,59 @@ def dirac2d4(sizes=(1024, 1024), nsteps=128) -> Workload:
     return Workload("dirac2d_4comp", tuple(sizes), dx, 1e-4, 4, nsteps, psi, V=V, note="harmonic well, 4 components")
 
 
+# ---------------------------------------------------------------------------------------------------------
+# the laser pulse of PAPER.md:400-412 (eq. 46a-c): inputs for the position-space vector-potential factor
+# ---------------------------------------------------------------------------------------------------------
+def pulse_envelope(eta, j: int, l: int):
+    """f_{j,l}(eta) of eq. 46c: j half cycles in all, linear turn-on and turn-off ramps of l half cycles each, plateau
+    in between, zero outside -j pi <= eta <= 0."""
+    eta = np.asarray(eta, dtype=np.float64)
+    x = eta / np.pi
+    f = np.zeros_like(eta)
+    on = (x >= -j) & (x <= -j + l)
+    flat = (x > -j + l) & (x < -l)
+    off = (x >= -l) & (x <= 0)
+    f[on] = (eta[on] + j * np.pi) / (l * np.pi)
+    f[flat] = 1.0
+    f[off] = -eta[off] / (l * np.pi)
+    return f
+
+
+def pulse_field(eta, E0: float, j: int, l: int):
+    """E(eta) = E0 sin(eta) f_{j,l}(eta), eta = k.x - omega t (eq. 46a); B = E / c (eq. 46b)."""
+    return E0 * np.sin(eta) * pulse_envelope(eta, j, l)
+
+
+def pulse_vector_potential(eta, E0: float, omega: float, j: int, l: int):
+    """A(eta) with E = -dA/dt = omega dA/deta and A = 0 ahead of the pulse (eta >= 0): A(eta) = -(1/omega) int_eta^0 E.
+    Closed form on each piece of the envelope: int sin(e) (a e + b) de = -(a e + b) cos(e) + a sin(e)."""
+    eta = np.asarray(eta, dtype=np.float64)
+
+    def F(e, a, b):  # antiderivative of sin(e) (a e + b)
+        return -(a * e + b) * np.cos(e) + a * np.sin(e)
+
+    pieces = [(-j * np.pi, (-j + l) * np.pi, 1.0 / (l * np.pi), j / l), ((-j + l) * np.pi, -l * np.pi, 0.0, 1.0),
+              (-l * np.pi, 0.0, -1.0 / (l * np.pi), 0.0)]
+    total = np.zeros_like(eta)  # int_eta^0 sin f
+    for lo, hi, a, b in pieces:
+        if hi <= lo:
+            continue
+        e0 = np.clip(eta, lo, hi)
+        total += F(hi, a, b) - F(e0, a, b)
+    return -(E0 / omega) * total
+
+
+def pulse_step_average(x, t: float, tau: float, E0: float, omega: float, j: int, l: int, kx: float):
+    """(1/tau) int_t^{t+tau} A(kx x - omega t') dt' by 8-point Gauss-Legendre quadrature (reading G12: the library and the
+    oracle are handed the same step average)."""
+    nodes, weights = np.polynomial.legendre.leggauss(8)
+    acc = np.zeros_like(np.asarray(x, dtype=np.float64))
+    for xi, wi in zip(nodes, weights):
+        tt = t + 0.5 * tau * (xi + 1.0)
+        acc += 0.5 * wi * pulse_vector_potential(kx * x - omega * tt, E0, omega, j, l)
+    return acc
+
+
 def random_state(sizes, ncomp, seed, dx=None) -> np.ndarray:
     """Unstructured complex Gaussian noise, normalised: the harshest parity input (all k populated)."""
     rng = np.random.default_rng(seed)
