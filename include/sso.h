@@ -139,8 +139,10 @@ int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nval
  * NULL switches the factor off.  Independent of SSO_FIELD_A, whose homogeneous A(t) enters the kinetic factor
  * (reading G16); the two splittings agree to O(tau^2).  ncomp = 1 gives SSO_ERR_UNSUPPORTED.  In this version the
  * factor runs as a kernel of its own where psi is in position space on every axis, i.e. before the first and after
- * the last pass of a step: while it is set, consecutive half steps are not merged (a 2D step costs an opening, a
- * kinetic and a closing pass plus two rotation kernels).  Synchronises `stream`.
+ * the last pass of a step: while it is set, consecutive potential half steps are not merged (a 2D step costs an
+ * opening, a kinetic and a closing pass) and the factor itself costs one kernel per step inside a call (the closing
+ * half of one step and the opening half of the next are one rotation) plus a half rotation at each end of the call.
+ * Synchronises `stream`.
  */
 int sso_set_vector_potential(sso_plan *plan, const double *A, int on_device, void *stream);
 

@@ -1692,7 +1692,7 @@ long long launches_for(const sso_plan *p, long long nsteps) {
     const bool kshift = p->ncomp == 1 && p->field_kind == SSO_FIELD_A;
     const bool kbuild = p->ncomp == 1 && (kshift || !p->kph_valid);
     if (p->ndim == 1) {
-        if (p->d_apos) return nsteps * 3;  // rotation, one step, rotation
+        if (p->d_apos) return 2 * nsteps + 1;  // rotation, then one step and one rotation per step
         if (cluster_size_for(p)) return kshift ? 2 * nsteps : 1 + (p->cl.kph_valid ? 0 : 1);
         if (kshift) return nsteps * (1 + p->ndim);
         return 1 + (kbuild ? p->ndim : 0);
@@ -1706,7 +1706,7 @@ long long launches_for(const sso_plan *p, long long nsteps) {
     cnt += nsteps * (p->ndim == 3 ? 3 : 1);      // kinetic sandwich (+ middle-axis DIF and DIT)
     if (dirac_split_kinetic(p)) cnt += 2 * nsteps;  // transform, pointwise factor, transform instead of one sandwich
     cnt += nsteps;                               // potential sandwiches and the closing pass
-    if (p->d_apos) cnt += 2 * nchunks;           // position-space rotations before every opening and after every closing pass
+    if (p->d_apos) cnt += nchunks + 1;           // position-space rotations: before the first opening pass, between chunks, after the last closing pass
     if (kshift) cnt += nsteps * p->ndim;
     else if (kbuild) cnt += p->ndim;
     return cnt;
@@ -1768,7 +1768,9 @@ static int step_impl(sso_plan *plan, void *psi, int64_t nsteps, void *stream, Ob
                 if ((rc = pass_status(plan, "1D cluster line kernel", lc(la, smem, st))) != SSO_OK) return rc;
                 continue;
             }
-            if ((rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
+            // position-space factor: half a step before the first step of the call, a whole one between two steps (the
+            // closing half of one and the opening half of the next use the same A), half a step after the last
+            if (s == 0 && (rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
             if (plan->ncomp == 1 && (rc = build_kphase(plan, n0 + s, st)) != SSO_OK) return rc;
             Line1dLaunchFn l1 = (plan->ncomp == 1 && plan->field_kind != SSO_FIELD_E) ? find_line1d(plan->precision, plan->ax[0].n) : nullptr;
             if (l1) {
@@ -1789,7 +1791,7 @@ static int step_impl(sso_plan *plan, void *psi, int64_t nsteps, void *stream, Ob
             }
             PassSpec ps{0, kpw, -1, 1, 1, 0, 1, 1, 1, (int)chunk, n0 + s};
             if ((rc = launch(plan, psi, ps, st)) != SSO_OK) return rc;
-            if ((rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
+            if ((rc = launch_rotation(plan, psi, s + chunk < nsteps ? 1.0 : 0.5, st)) != SSO_OK) return rc;
         }
     } else {
         // chunks that share one set of field phase rows; each chunk opens and closes with a half step
@@ -1804,7 +1806,8 @@ static int step_impl(sso_plan *plan, void *psi, int64_t nsteps, void *stream, Ob
             const long long nb = n0 + c0;
             if ((rc = build_erows(plan, nb, ns, st)) != SSO_OK) return rc;
             // opening: V/2 in natural order, forward transform along the last axis, natural frequency order out
-            if ((rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
+            // (position-space factor: half a step before the first chunk, a whole one between chunks, half after the last)
+            if (c0 == 0 && (rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
             if ((rc = launch_ring_pass(plan, psi, MODE_OPEN, 0, st)) != SSO_OK) return rc;
             for (long long s = 0; s < ns; ++s) {
                 const long long n = nb + s;
@@ -1851,7 +1854,7 @@ static int step_impl(sso_plan *plan, void *psi, int64_t nsteps, void *stream, Ob
                 if (ob && fused) *fused = true;
                 if ((rc = launch_ring_pass(plan, psi, s + 1 < ns ? MODE_MID : MODE_CLOSE, s + 1, st, ob)) != SSO_OK) return rc;
             }
-            if ((rc = launch_rotation(plan, psi, 0.5, st)) != SSO_OK) return rc;
+            if ((rc = launch_rotation(plan, psi, c0 + ns < nsteps ? 1.0 : 0.5, st)) != SSO_OK) return rc;
         }
     }
     plan->tindex += nsteps;
