@@ -9,7 +9,7 @@ sso_step(psi, SPLIT_STEPS) that advances the wavefunction by SPLIT_STEPS = 128 s
 
 Headline workload at N=1: BASELINE.json's metric is not quoted on one config, so the line's top-level numbers are
 for the LARGEST single-GPU configuration, config 5 (3D Dirac, 4 x 256^3 complex128, 1 GiB of psi); the other
-workloads (1, 2a, 2b, 3, 4, and the paper's 1D Dirac and 4-component 2D Dirac shapes d1, d2x4) are timed in the same run and reported under config.per_workload.
+workloads (1, 2a, 2b, 3, 4, and the paper's 1D Dirac and 4-component 2D Dirac shapes d1, d2x4, d2A) are timed in the same run and reported under config.per_workload.
   value  device-resident throughput: psi, the potential table and the field table are in HBM before the
          timed region; K calls timed with CUDA events on the launching stream.
   e2e    the same K calls through sso_step_host on a pinned HOST buffer: every call uploads psi, steps and
@@ -53,6 +53,8 @@ WORKLOADS = {
     "1": (1, "c128", 1), "2a": (2, "c128", 2), "2b": (2, "c64", 2), "3": (3, "c128", 4), "4": (4, "c128", 2), "5": (5, "c128", 4),
     # the paper's own remaining shapes: 1D Dirac (eq. 35) and 2D Dirac with all four components
     "d1": ("dirac1d", "c128", 1), "d2x4": ("dirac2d4", "c128", 2),
+    # the paper's position-space interaction factor (eq. 26): opening, kinetic, closing pass + one rotation kernel per step
+    "d2A": ("dirac2dA", "c128", 4),
 }
 DESCR = {
     "1": "cfg1 1D Schroedinger 4096, harmonic well, complex128",
@@ -63,10 +65,11 @@ DESCR = {
     "5": "cfg5 3D Dirac 4 components 256^3, soft-core Coulomb, complex128",
     "d1": "1D Dirac 2 components 4096 (PAPER.md:240 eq. 35), soft-core well zeta=1.4133, complex128",
     "d2x4": "2D Dirac 4 components 1024x1024 (the paper's 2D code, PAPER.md:115, 310), harmonic well, complex128",
+    "d2A": "2D Dirac 2 components 1024x1024 with A(r) of a magnetic field applied in position space (PAPER.md:198 eq. 26), complex128",
 }
 # 60 % of the 8 TB/s roofline, us per split step; None where the bar does not apply
 OPTIONS = []  # (SSO_OPT_*, value) pairs from --opt, applied to every plan (tuning sweeps)
-BAR_US = {"1": None, "2a": 55.9, "2b": 28.0, "3": 447.4, "4": 28.0, "5": 1789.6, "d1": None, "d2x4": 55.9}
+BAR_US = {"1": None, "2a": 55.9, "2b": 28.0, "3": 447.4, "4": 28.0, "5": 1789.6, "d1": None, "d2x4": 55.9, "d2A": None}
 
 
 def load_peaks():
@@ -108,6 +111,8 @@ def make_workload(name: str, nrows: int):
         w = wl.dirac1d(sizes=(4096,), nsteps=nrows, ncomp=2)
     elif cfg == "dirac2d4":
         w = wl.dirac2d4(nsteps=nrows)
+    elif cfg == "dirac2dA":
+        w = wl.dirac2d_magnetic(nsteps=nrows)
     else:
         w = wl.CONFIGS[cfg](nsteps=nrows)
     return w, prec, P
@@ -174,6 +179,8 @@ def oracle_rate(w, seconds_target: float, threads: int | None = None):
         o.set_potential(w.V)
         if w.field_kind:
             o.set_field(w.field_kind, w.step_avg)
+        if "A" in w.extra:
+            o.set_vector_potential(w.extra["A"])
         psi = w.psi0
         t0 = time.perf_counter()
         psi = o.step(psi, 1)
@@ -199,12 +206,14 @@ def run_reference(args):
     import oracle
 
     name = args.workload
-    REF_SPLIT = {"1": 128, "2a": 4, "2b": 4, "3": 1, "4": 8, "5": 1, "d1": 128, "d2x4": 2}[name]
+    REF_SPLIT = {"1": 128, "2a": 4, "2b": 4, "3": 1, "4": 8, "5": 1, "d1": 128, "d2x4": 2, "d2A": 4}[name]
     w, prec, P = make_workload(name, REF_SPLIT * (args.steps + args.warmup) + 1)
     o = oracle.Solver(w.sizes, w.dx, w.dt, w.ncomp, w.mass, w.c, w.charge)
     o.set_potential(w.V)
     if w.field_kind:
         o.set_field(w.field_kind, w.step_avg)
+    if "A" in w.extra:
+        o.set_vector_potential(w.extra["A"])
     psi = w.psi0 if prec == "c128" else w.psi0.astype(np.complex64).astype(np.complex128)
     for _ in range(args.warmup):
         psi = o.step(psi, REF_SPLIT)
@@ -260,6 +269,8 @@ def measure(name, K, W, world, barrier, sampler, want_e2e):
     plan.set_potential(w.V)
     if w.field_kind:
         plan.set_field(w.field_kind, np.ascontiguousarray(w.step_avg))
+    if "A" in w.extra:
+        plan.set_vector_potential(np.ascontiguousarray(w.extra["A"]))
     psi0 = w.psi0.astype(cdt)
     psi = torch.from_numpy(psi0).cuda()
     stream = torch.cuda.current_stream()

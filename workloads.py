@@ -230,6 +230,21 @@ def dirac2d4(sizes=(1024, 1024), nsteps=128) -> Workload:
     return Workload("dirac2d_4comp", tuple(sizes), dx, 1e-4, 4, nsteps, psi, V=V, note="harmonic well, 4 components")
 
 
+def dirac2d_magnetic(sizes=(1024, 1024), nsteps=128) -> Workload:
+    """2D Dirac, 2 components, with a POSITION-DEPENDENT vector potential applied in position space as the paper does
+    (eq. 18a, 188-198 eq. 26): homogeneous magnetic field B = 50 a.u. in the symmetric gauge
+    A = (B/2)(-y, x), soft-core well, positive-energy packet.  extra["A"] holds A(r), shape (2, *sizes)."""
+    rng = np.random.default_rng(SEED0 + 8)
+    dx = (0.1, 0.1)
+    X, Y = mesh(sizes, dx)
+    V = -1.0 / np.sqrt(X**2 + Y**2 + 0.791**2)
+    kbar = rng.uniform(-5.0, 5.0, size=2)
+    psi = dirac_packet(sizes, dx, kbar, 1.0, 2, 1.0, C_LIGHT)
+    B = 50.0
+    A = np.stack([-0.5 * B * Y, 0.5 * B * X])
+    return Workload("dirac2d_magnetic", tuple(sizes), dx, 1e-4, 2, nsteps, psi, V=V, note="B = 50 a.u., symmetric gauge", extra={"A": A})
+
+
 # ---------------------------------------------------------------------------------------------------------
 # the laser pulse of PAPER.md:400-412 (eq. 46a-c): inputs for the position-space vector-potential factor
 # ---------------------------------------------------------------------------------------------------------
