@@ -1368,9 +1368,11 @@ SRingShape sring_shape(const sso_plan *plan, int axis, int cc, bool light) {
     } else {
         // the widest rows (up to 128 bytes; 256 bytes for the transform-only passes, measured 393 -> 336 us per pass
         // on config 5) that leave room for two buffers or more
+        // (16-byte rows only when nothing wider fits at all: the 4-component 1024-point Dirac tile measured 80.7 us per
+        // pass with two buffers of 16-byte rows, 76.2 with one buffer of 32-byte rows)
         for (int want = 2; want >= 1 && !TL; --want)
             for (int cand = light ? 2 * Gn : Gn; cand >= 1 && !TL; cand /= 2)
-                if (fits(cand, &bm) && bm >= want) TL = cand;
+                if (fits(cand, &bm) && bm >= want && (want == 1 || cand * esz >= 32)) TL = cand;
     }
     if (!TL) return r;
     r.TL = TL;
