@@ -1075,7 +1075,7 @@ int tile_order_mask(const sso_plan *p) {
 }
 
 // Every ring pass reserves 512 bytes of shared memory behind its buffers: the pool state of sso_ring.cuh (TileRing::bytes:
-// 12 NB + 136 + 4 G <= 340 for NB <= 12, G <= 15) and, from byte 448, the observable sums of the closing pass.
+// 16 NB + 8 + 4 G <= 260 for NB <= 12, G <= 15) and, from byte 448, the observable sums of the closing pass.
 
 // lines per component per CTA
 int choose_tl(const sso_plan *p, const Geometry &g, int cc) {

@@ -96,18 +96,19 @@ __device__ __forceinline__ void prefetch_l2_bulk_plain(const void *p, unsigned b
 // Tile buffers of a persistent CTA: NB shared-memory buffers shared by G compute groups (NB >= G).  The CTA's tiles
 // 0 .. nloc-1 are loaded in that order, each into whichever buffer is free: the first NB go to buffers 0 .. NB-1,
 // and every time a group has emptied a buffer its leader claims the next unloaded tile for it.  Groups consume the
-// tiles in the same order: a leader draws a ticket s (= the s-th tile of the CTA) from a counter, looks up which
-// buffer that tile went to, and the group waits for it there.  With NB > G the spare buffers hold tiles that are
-// loading or ready while all groups compute, so a group that finishes finds its next tile already on chip; with
-// NB = G a group simply gets back the buffer it refilled.
-// A waiter cannot be a fill ahead of its barrier's phase: the slot of tile s names the buffer AND the parity of the
-// fill, and it is published only when that fill is issued, i.e. after the buffer's previous fill has been consumed.
-// (A fixed ticket -> buffer map does not have that property: a group can lap a slow one and wait on a buffer whose
-// previous fill has not even landed, and the parity of its wait then matches a phase that is two fills old.)
+// tiles in the same order: a leader draws a ticket s (= the s-th tile of the CTA) from a counter, and the group looks
+// for the buffer that holds tile s (every buffer carries the number of its tile and the parity of its fill, written
+// when the fill is issued) and waits for it there.  With NB > G the spare buffers hold tiles that are loading or
+// ready while all groups compute, so a group that finishes finds its next tile already on chip; with NB = G a group
+// simply gets back the buffer it refilled.
+// A waiter cannot be a fill ahead of its barrier's phase: a buffer is tagged with tile s only when that fill is issued,
+// i.e. after the buffer's previous fill has been consumed, and it keeps the tag until the group that drew ticket s has
+// worked on it -- however long that group takes.  (A fixed ticket -> buffer map does not have that property: a group
+// can lap a slow one and wait on a buffer whose previous fill has not even landed, and the parity of its wait then
+// matches a phase that is two fills old.  tests/test_tile_pool_protocol.py is a model of both.)
 struct TileRing {
-    static constexpr int QN = 32;  // slots in flight: more than NB + G
     unsigned long long *bar;  // [NB] "tile landed" barriers
-    volatile int *slot;       // [QN] slot[s % QN] = (s + 1) << 8 | parity << 7 | buffer, written when tile s is issued
+    volatile int *tag;        // [NB] tag[b] = (tile + 1) << 1 | parity of the fill that brings it, 0: never filled
     volatile int *fills;      // [NB] fills issued into each buffer so far
     int *next;                // next unloaded tile of the CTA
     int *ticket;              // next ticket
@@ -115,13 +116,13 @@ struct TileRing {
     int NB, G;
     __device__ TileRing(void *base, int nb, int g) : NB(nb), G(g) {
         bar = reinterpret_cast<unsigned long long *>(base);
-        slot = reinterpret_cast<volatile int *>(bar + nb);
-        fills = slot + QN;
+        tag = reinterpret_cast<volatile int *>(bar + nb);
+        fills = tag + nb;
         next = const_cast<int *>(fills) + nb;
         ticket = next + 1;
         mail = ticket + 1;
     }
-    static __host__ __device__ size_t bytes(int nb, int g) { return (size_t)nb * 12 + QN * 4 + 8 + (size_t)g * 4; }
+    static __host__ __device__ size_t bytes(int nb, int g) { return (size_t)nb * 16 + 8 + (size_t)g * 4; }
     __device__ void *full(int b) const { return bar + b; }
     // once per CTA, by thread 0, before the __syncthreads that precedes the first fill
     __device__ void init() const {
@@ -129,31 +130,35 @@ struct TileRing {
             for (int b = 0; b < NB; ++b) {
                 mbar_init(bar + b, 1);
                 fills[b] = 0;
+                tag[b] = 0;
             }
-            for (int q = 0; q < QN; ++q) slot[q] = 0;
             *next = NB;  // tiles 0 .. NB-1 go to buffers 0 .. NB-1
             *ticket = 0;
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
     }
-    // by the thread that issues the load of tile s into buffer b (one issuer per buffer at a time): publish where
-    // tile s lands; the caller arms the barrier and starts the copy
+    // by the thread that issues the load of tile s into buffer b (one issuer per buffer at a time): tag the buffer;
+    // the caller arms the barrier and starts the copy
     __device__ void publish(int s, int b) const {
         const int f = fills[b];
         fills[b] = f + 1;
-        const int par = f & 1;
-        slot[s % QN] = ((s + 1) << 8) | (par << 7) | b;
+        tag[b] = ((s + 1) << 1) | (f & 1);
     }
     // group leader: draw the group's next ticket; the group barrier that follows publishes it
     __device__ void draw(int grp) const { mail[grp] = atomicAdd(ticket, 1); }
     __device__ int drawn(int grp) const { return mail[grp]; }
     // blocks until tile s (< nloc) has landed; returns its buffer
     __device__ int wait(int s) const {
-        int v;
-        while (((v = slot[s % QN]) >> 8) != s + 1) __nanosleep(64);
-        const int b = v & 127;
-        mbar_wait(bar + b, (unsigned)((v >> 7) & 1));
-        return b;
+        for (;;) {
+            for (int b = 0; b < NB; ++b) {
+                const int v = tag[b];
+                if ((v >> 1) == s + 1) {
+                    mbar_wait(bar + b, (unsigned)(v & 1));
+                    return b;
+                }
+            }
+            __nanosleep(64);  // the load of tile s has not been issued yet
+        }
     }
     __device__ int claim() const { return atomicAdd(next, 1); }
 };
