@@ -396,20 +396,19 @@ __global__ void __launch_bounds__(MAXT, 1) ring_kernel(const RingArgs a) {
         }
     }
     if constexpr (OBS) {
-        // warp sums by shuffles, CTA sums by shared-memory atomics, one row of partial sums per CTA (a final kernel adds
+        // CTA sums by shared-memory atomics, one row of partial sums per CTA (a final kernel adds
         // the rows in a fixed order; which tiles a warp met depends on the tile pool, so the last bits may differ from run to run)
         double *cta = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(bufs + (size_t)a.NB * a.bufstride) + 448);
         __syncthreads();  // every group has left the tile loop
-        if (threadIdx.x < 6) cta[threadIdx.x] = 0.0;
+        if (threadIdx.x == 0)  // (a CTA of a tiny lattice may have fewer than six threads)
+            for (int v = 0; v < 6; ++v) cta[v] = 0.0;
         __syncthreads();
+        // (a CTA of a tiny lattice may hold a partial warp, so no full-mask shuffles here: once per launch, the cost is nil)
 #pragma unroll
-        for (int v = 0; v < 6; ++v) {
-            double s = ob[v];
-            for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
-            if ((threadIdx.x & 31) == 0) atomicAdd(&cta[v], s);
-        }
+        for (int v = 0; v < 6; ++v) atomicAdd(&cta[v], ob[v]);
         __syncthreads();
-        if (threadIdx.x < 6) a.obs_partial[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = cta[threadIdx.x];
+        if (threadIdx.x == 0)
+            for (int v = 0; v < 6; ++v) a.obs_partial[(size_t)v * gridDim.x + blockIdx.x] = cta[v];
     }
 }
 
