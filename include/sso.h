@@ -38,7 +38,7 @@
  * Error behaviour: every function returns an int status (0 = SSO_OK); nothing is
  * thrown across the ABI.  sso_last_error(plan) returns a plan-owned, NUL-terminated
  * description of the most recent failure on that plan (or, for plan == NULL, of the
- * most recent failed sso_plan_create on this thread).
+ * most recent failed sso_plan_create or sso_norm_static on this thread).
  */
 #ifndef SSO_H_
 #define SSO_H_
@@ -173,6 +173,43 @@ int sso_step_host(sso_plan *plan, void *psi_host, int64_t nsteps);
  * accumulated in double also for SSO_C64, in a fixed order (deterministic).  Synchronises `stream`.
  */
 int sso_norm(sso_plan *plan, const void *psi, double *out_host, void *stream);
+
+/*
+ * The same norm for callers that cannot allocate device memory -- no plan, no cudaMalloc, no cudaFree, no call into
+ * an allocating library, on any call.  Meant for: a process whose own arena (or the framework around it) already
+ * owns all of HBM, where an allocation made by this library would simply fail; a time loop that must not stall,
+ * since cudaMalloc and cudaFree wait for everything running on the device; a monitor that is handed a pointer to a
+ * wavefunction some other component propagates and has no plan of its own (creating one allocates tables).
+ *
+ *   *out_dev = vol * sum_{i < count} |psi[i]|^2        (the quantity of sso_norm; eq. 7, 76 eq. 8, 331)
+ *
+ * psi      DEVICE pointer to `count` complex numbers (all components and lattice points of the state, any lattice
+ *          shape), float2 for SSO_C64 or double2 for SSO_C128, aligned to one complex number; caller-owned, read only.
+ * vol      prod(dx) of the lattice (there is no plan to take it from); finite.
+ * out_dev  DEVICE pointer to one double, 8-byte aligned, caller-owned; written by the last kernel of the call.
+ * stream   the two kernels are enqueued on it; the call does not wait for them and copies nothing to the host.
+ *
+ * The per-chunk partial sums (one per SSO_NORM_STATIC_CHUNK elements, accumulated in double in a fixed order, so the
+ * result is deterministic and does not depend on the GPU model) go to an array built into the library image, of
+ * SSO_NORM_STATIC_MAX_COUNT / SSO_NORM_STATIC_CHUNK doubles = 256 KiB; every GPU that loads libsso.so holds it until
+ * the process exits.  Hence the limit: count > SSO_NORM_STATIC_MAX_COUNT returns SSO_ERR_INVALID (split the state
+ * and add the pieces, or use sso_norm).  count = 0 gives *out_dev = 0.
+ *
+ * All calls on a device share that one array, and it keeps what the last call left in it.  A call overwrites every
+ * slot it later reads, so nothing needs clearing between calls -- but two calls whose kernels can overlap on the
+ * GPU (different streams without an ordering between them, or two host threads) race on it and may both return
+ * garbage; order them with events or keep them on one stream.  Different devices have separate copies.
+ *
+ * The first call on each device (with that device current, as for every call) also looks up the array's address
+ * on that device, which can make the CUDA runtime load the library's device code there.  Make that first call
+ * during set-up, before starting any stream capture.  Later calls only launch the two kernels.
+ *
+ * Errors are reported through sso_last_error(NULL), like those of sso_plan_create.  The value agrees with sso_norm
+ * to rounding (the order of the additions differs), not bit for bit.
+ */
+#define SSO_NORM_STATIC_CHUNK 8192                 /* complex numbers summed into one partial sum           */
+#define SSO_NORM_STATIC_MAX_COUNT (1LL << 28)      /* largest count per call (4 GiB of complex128)          */
+int sso_norm_static(const void *psi, int precision, int64_t count, double vol, double *out_dev, void *stream);
 
 /*
  * Observables (section V.2).  psi, psi_a, psi_b are DEVICE pointers laid out as for sso_step, in

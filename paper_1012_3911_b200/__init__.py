@@ -29,9 +29,10 @@ SYMBOLS = (
     "sso_get_time_index", "sso_step", "sso_step_host", "sso_norm", "sso_set_option", "sso_launch_count",
     "sso_destroy", "sso_last_error", "sso_version", "sso_debug_layout", "sso_profile_step", "sso_pass_name",
     "sso_set_vector_potential", "sso_overlap", "sso_expect_position", "sso_expect_momentum", "sso_spectrum",
-    "sso_filter_accumulate", "sso_step_observe",
+    "sso_filter_accumulate", "sso_step_observe", "sso_norm_static",
 )
 PASS_KINDS = 9
+NORM_STATIC_CHUNK, NORM_STATIC_MAX_COUNT = 8192, 1 << 28  # SSO_NORM_STATIC_* of include/sso.h
 
 
 class SsoError(RuntimeError):
@@ -76,6 +77,7 @@ def lib() -> ctypes.CDLL:
         L.sso_filter_accumulate.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp]
         L.sso_step_observe.argtypes = [vp, vp, i64, vp, vp, dbl, dbl, dbl, dbl, ctypes.POINTER(dbl), vp]
         L.sso_pass_name.restype = ctypes.c_char_p
+        L.sso_norm_static.argtypes = [vp, ci, i64, dbl, vp, vp]
         for name in SYMBOLS:
             if name not in ("sso_last_error", "sso_version", "sso_pass_name"):
                 getattr(L, name).restype = ci
@@ -131,6 +133,37 @@ def _stream(s) -> Optional[int]:
     if isinstance(s, int):
         return s or None
     return s.cuda_stream  # torch.cuda.Stream
+
+
+def norm_static(psi, vol: float, out, precision: Optional[int] = None, count: Optional[int] = None, stream=None) -> None:
+    """``sso_norm_static``: out[0] = vol * sum |psi|^2 for callers that must not allocate device memory.
+
+    No plan is involved and the library calls neither cudaMalloc nor cudaFree: the partial sums go to an array
+    built into libsso.so (256 KiB per GPU, which is why ``count`` may not exceed ``NORM_STATIC_MAX_COUNT``).  Use it
+    when the application's arena already owns all of HBM, when the time loop cannot afford the device-wide wait of
+    an allocation, or when there is only a pointer to somebody else's wavefunction and no plan.  ``psi`` is a
+    contiguous CUDA tensor of complex64/complex128 (or a raw device address, then ``precision`` and ``count`` are
+    required), ``out`` a CUDA float64 tensor with at least one element (or a raw address) that receives the result;
+    the caller allocates both.  Nothing is synchronised or copied to the host: read ``out`` after the stream has
+    finished.  All calls on a device share the built-in array, so calls whose kernels could overlap on the GPU must
+    be ordered by the caller; make the first call on a device during set-up (it resolves the array's address).
+    """
+    if hasattr(psi, "data_ptr"):
+        if not psi.is_cuda or not psi.is_contiguous():
+            raise ValueError("psi: expected a contiguous CUDA tensor")
+        if not psi.is_complex():
+            raise ValueError("psi: expected a complex64 or complex128 tensor")
+        if precision is None:
+            precision = C128 if psi.element_size() == 16 else C64
+        if count is None:
+            count = psi.numel()
+    if precision is None or count is None:
+        raise ValueError("precision and count are required with a raw psi address")
+    if hasattr(out, "data_ptr") and (not out.is_cuda or out.element_size() != 8 or out.numel() < 1):
+        raise ValueError("out: expected a CUDA float64 tensor with at least one element")
+    rc = lib().sso_norm_static(_ptr(psi), int(precision), int(count), float(vol), _ptr(out), _stream(stream))
+    if rc != OK:
+        raise SsoError(rc, (lib().sso_last_error(None) or b"").decode())
 
 
 class Plan:

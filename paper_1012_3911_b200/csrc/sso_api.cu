@@ -17,6 +17,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -2080,3 +2081,105 @@ int sso_step_observe(sso_plan *plan, void *psi, int64_t nsteps, const void *psi_
 }
 
 }  // extern "C"
+
+// ---- sso_norm_static: the norm for callers that cannot allocate device memory ---------------------------------------
+//
+// sso_norm keeps its per-CTA partial sums in a buffer that sso_plan_create obtained with cudaMalloc.  Some callers
+// cannot get that far: the application (or the framework it runs in) has handed the whole of HBM to an arena of its
+// own, so a cudaMalloc from this library would fail; or the caller sits in a time loop that must not stall, and
+// cudaMalloc / cudaFree wait for all work on the device; or it only holds a pointer to a wavefunction another
+// component propagates and has no plan (every plan allocates tables).  For them the partial sums live in the array
+// below.  It is part of the library image: every GPU that loads libsso.so holds these 256 KiB until the process
+// exits, whether or not this entry point is ever called.
+//
+// In host code `g_norm_static_partial` is only a handle for the runtime, not a device address; the address on the
+// current device comes from cudaGetSymbolAddress (norm_static_scratch below), once per device.
+static __device__ __align__(256) double g_norm_static_partial[SSO_NORM_STATIC_MAX_COUNT / SSO_NORM_STATIC_CHUNK];
+
+namespace {
+
+constexpr int NORM_STATIC_THREADS = 256;
+constexpr int NORM_STATIC_MAX_DEVICES = 64;
+
+// CTA b sums |psi|^2 over elements [b * CHUNK, min(count, (b+1) * CHUNK)) in double, in a fixed order, and writes
+// partial[b].  One partial per chunk of the input (not per resident CTA as in norm_partial_kernel): the sum does not
+// depend on the SM count of the device.
+template <typename T>
+__global__ void __launch_bounds__(NORM_STATIC_THREADS) norm_static_partial_kernel(const void *__restrict__ psi, long long count, double *__restrict__ partial) {
+    using C = typename Cx2<T>::type;
+    const C *p = reinterpret_cast<const C *>(psi);
+    const long long lo = (long long)blockIdx.x * SSO_NORM_STATIC_CHUNK;
+    const long long hi = lo + SSO_NORM_STATIC_CHUNK < count ? lo + SSO_NORM_STATIC_CHUNK : count;
+    double acc = 0.0;
+#pragma unroll 8
+    for (long long i = lo + threadIdx.x; i < hi; i += NORM_STATIC_THREADS) {
+        const C v = p[i];
+        acc += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
+    }
+    double a[1] = {acc};
+    block_sum<1>(a);
+    if (threadIdx.x == 0) partial[blockIdx.x] = a[0];
+}
+
+// *out = vol * sum_{b < n} partial[b]; one CTA, fixed order.  Reads only the n slots the launch before it wrote.
+__global__ void __launch_bounds__(1024) norm_static_final_kernel(const double *__restrict__ partial, int n, double vol, double *__restrict__ out) {
+    double a[1] = {0.0};
+    for (int i = threadIdx.x; i < n; i += blockDim.x) a[0] += partial[i];
+    block_sum<1>(a);
+    if (threadIdx.x == 0) *out = a[0] * vol;
+}
+
+// Device address of g_norm_static_partial on the CURRENT device; looked up on the first call per device, then cached.
+// The look-up may make the runtime load the library's device code onto that device; it allocates nothing of ours.
+static cudaError_t norm_static_scratch(double **ptr, int *device) {
+    static double *cached[NORM_STATIC_MAX_DEVICES] = {};
+    static std::mutex mu;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    *device = dev;
+    if (dev < 0 || dev >= NORM_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!cached[dev]) {
+        double *p = nullptr;
+        e = cudaGetSymbolAddress((void **)&p, g_norm_static_partial);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        cached[dev] = p;
+    }
+    *ptr = cached[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int sso_norm_static(const void *psi, int precision, int64_t count, double vol, double *out_dev, void *stream) {
+    sso_plan *plan = nullptr;  // errors are reported like those of sso_plan_create: sso_last_error(NULL)
+    if (precision != SSO_C64 && precision != SSO_C128) return fail(nullptr, SSO_ERR_INVALID, "sso_norm_static: precision must be SSO_C64 or SSO_C128");
+    if (count < 0) return fail(nullptr, SSO_ERR_INVALID, "sso_norm_static: count must be >= 0");
+    if (count > SSO_NORM_STATIC_MAX_COUNT)
+        return fail(nullptr, SSO_ERR_INVALID,
+                    "sso_norm_static: count " + std::to_string((long long)count) + " exceeds SSO_NORM_STATIC_MAX_COUNT = " +
+                        std::to_string((long long)SSO_NORM_STATIC_MAX_COUNT) +
+                        " complex numbers (the built-in scratch array holds one partial sum per " + std::to_string(SSO_NORM_STATIC_CHUNK) +
+                        " of them); use sso_norm with a plan, or call once per piece and add the results");
+    if (!out_dev) return fail(nullptr, SSO_ERR_INVALID, "sso_norm_static: out_dev is NULL");
+    if (!psi && count > 0) return fail(nullptr, SSO_ERR_INVALID, "sso_norm_static: psi is NULL");
+    if (!isfinite(vol)) return fail(nullptr, SSO_ERR_INVALID, "sso_norm_static: vol must be finite");
+    const uintptr_t align = precision == SSO_C128 ? 16 : 8;
+    if (((uintptr_t)psi % align) != 0 || ((uintptr_t)out_dev % 8) != 0) return fail(nullptr, SSO_ERR_INVALID, "sso_norm_static: psi must be aligned to one complex number, out_dev to 8 bytes");
+    double *scratch = nullptr;
+    int dev = -1;
+    cudaError_t e = norm_static_scratch(&scratch, &dev);
+    if (e != cudaSuccess) return fail(nullptr, SSO_ERR_CUDA, "sso_norm_static: address of the scratch array on device " + std::to_string(dev) + ": " + cudaGetErrorString(e));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int nchunks = (int)((count + SSO_NORM_STATIC_CHUNK - 1) / SSO_NORM_STATIC_CHUNK);
+    // nothing in the scratch array has to start at zero: this call writes slots [0, nchunks) and reads only those
+    if (nchunks > 0) {
+        if (precision == SSO_C128) norm_static_partial_kernel<double><<<nchunks, NORM_STATIC_THREADS, 0, st>>>(psi, count, scratch);
+        else norm_static_partial_kernel<float><<<nchunks, NORM_STATIC_THREADS, 0, st>>>(psi, count, scratch);
+    }
+    norm_static_final_kernel<<<1, 1024, 0, st>>>(scratch, nchunks, vol, out_dev);
+    CK(cudaGetLastError());
+    return SSO_OK;
+}
