@@ -72,19 +72,18 @@ extern "C" {
                                             no copy of V: CHANGING this option discards the potential,
                                             and sso_step fails with SSO_ERR_STATE until
                                             sso_set_potential has been called again                */
-
 #define SSO_OPT_GROUPS_PER_CTA 4         /* independent line groups per CTA (0 = auto)              */
 #define SSO_OPT_RING_BUFFERS 5           /* tile buffers per CTA of the pass pipelines (0 = auto: as many as fit)  */
+#define SSO_OPT_THREADS_PER_CTA 6        /* ring pipeline CTA size: 512 (128 regs/thread) or 384 (168); 0 = auto */
 #define SSO_OPT_STRIDED_RING 7           /* strided-axis passes: 0 auto, 1 force the TMA ring, 2 direct kernel only */
 #define SSO_OPT_DIRAC_TABLE 8            /* Dirac plans without a field, ndim >= 2: 0 = cos(E tau), sin(E tau)/E of every k point
                                             evaluated in the kinetic pass, 1 = read from a table (16 bytes per k point) */
-#define SSO_OPT_LINES_PER_TILE_MIDDLE 10 /* adjacent lines per tile in the middle-axis passes of a 3D lattice (0 = auto)  */
-#define SSO_OPT_CLUSTER_1D 11            /* 1D Schroedinger steps on a thread-block cluster: 0 = auto, 1 = off (single CTA; lattices
-                                            beyond SSO_MAX_AXIS then fail), 4 or 8 = CTAs per cluster (needs sizes[0]/value in [512, 4096]) */
 #define SSO_OPT_TILE_ORDER 9              /* order in which the passes walk their tiles: 0 = auto; otherwise value - 1 is a mask of
                                             the passes that go from the highest address down (bit 0 contiguous-axis passes,
                                             1 middle-axis forward, 2 middle-axis inverse, 3 kinetic); results do not depend on it */
-#define SSO_OPT_THREADS_PER_CTA 6        /* ring pipeline CTA size: 512 (128 regs/thread) or 384 (168); 0 = auto */
+#define SSO_OPT_LINES_PER_TILE_MIDDLE 10 /* adjacent lines per tile in the middle-axis passes of a 3D lattice (0 = auto)  */
+#define SSO_OPT_CLUSTER_1D 11            /* 1D Schroedinger steps on a thread-block cluster: 0 = auto, 1 = off (single CTA; lattices
+                                            beyond SSO_MAX_AXIS then fail), 4 or 8 = CTAs per cluster (needs sizes[0]/value in [512, 4096]) */
 
 #define SSO_MIN_AXIS 16   /* smallest supported axis length                       */
 #define SSO_MAX_AXIS 8192 /* largest supported axis length: one CTA of 512 threads holds a line (16 points per thread) */
@@ -135,7 +134,8 @@ int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nval
  * (eq. 23/24; with q = -1 this is eq. 26 as printed; eq. 34, in
  * one dimension).  A is the STEP AVERAGE of the field on the lattice (its time integral over a step divided by
  * tau, reading G12), double[ndim][n0][n1][n2] in C order, host or device pointer; copied, the caller keeps
- * ownership; it is used for every following step until replaced (a time-dependent A(r,t) is set step by step);
+ * ownership; a HOST array is checked for non-finite values (SSO_ERR_INVALID), a DEVICE array is not (a NaN there ends
+ * up in psi: the caller's responsibility); it is used for every following step until replaced (a time-dependent A(r,t) is set step by step);
  * NULL switches the factor off.  Independent of SSO_FIELD_A, whose homogeneous A(t) enters the kinetic factor
  * (reading G16); the two splittings agree to O(tau^2).  ncomp = 1 gives SSO_ERR_UNSUPPORTED.  In this version the
  * factor runs as a kernel of its own where psi is in position space on every axis, i.e. before the first and after
@@ -154,8 +154,13 @@ int sso_get_time_index(const sso_plan *plan, int64_t *n);
  * Advance psi in place by nsteps >= 0 steps.  psi is a DEVICE pointer to
  * ncomp * prod(sizes) complex numbers in the plan's precision, 16-byte aligned;
  * the caller owns it.  Asynchronous on `stream`; only kernels are enqueued (the
- * call can be captured into a CUDA graph).  Consecutive potential half steps
- * inside one call are merged into one phase (identical up to rounding).
+ * call can be captured into a CUDA graph), from the first call on: every device
+ * table whose shape depends on the configuration is (re)allocated by the call that
+ * sets the configuration (sso_plan_create, sso_set_option, sso_set_field,
+ * sso_set_potential, sso_set_vector_potential), never by sso_step; if such an
+ * allocation failed there, sso_step returns SSO_ERR_STATE instead of allocating.
+ * Consecutive potential half steps inside one call are merged into one phase
+ * (identical up to rounding).
  */
 int sso_step(sso_plan *plan, void *psi, int64_t nsteps, void *stream);
 
@@ -222,7 +227,8 @@ int sso_norm_static(const void *psi, int precision, int64_t count, double vol, d
  * sso_expect_position: out_host[a] = sum r_a |psi|^2 prod(dx), a < ndim, on the grid r_j = (j - n/2) dx (reading G14).
  * sso_expect_momentum: out_host[a] = sum_k k_a |psi~(k)|^2 prod(dx) / N, the canonical momentum (hbar = 1), psi~ the
  *   unnormalised forward transform of PAPER.md:103 eq. 12 taken on a plan-owned copy (psi is not modified; the copy
- *   is allocated on first use and costs as much device memory as psi).
+ *   is allocated on first use and costs as much device memory as psi).  Axes of at most SSO_MAX_AXIS points: for a
+ *   longer 1D lattice (SSO_MAX_AXIS_1D) the call returns SSO_ERR_UNSUPPORTED before it allocates or enqueues anything.
  */
 int sso_overlap(sso_plan *plan, const void *psi_a, const void *psi_b, double *out_host, void *stream);
 int sso_expect_position(sso_plan *plan, const void *psi, double *out_host, void *stream);
@@ -296,13 +302,6 @@ const char *sso_pass_name(int kind);
 int sso_destroy(sso_plan *plan);
 
 const char *sso_last_error(const sso_plan *plan);
-
-/*
- * Host-only introspection of the plan builder (no GPU needed; used by the CPU tests): for a line of n points,
- * pos_freq[p] = frequency index held at position p after the decimation-in-frequency stages, and
- * slot_nat[s] = natural index stored at slot s of the permuted table layout.  Both are host int[n].
- */
-int sso_debug_layout(int n, int *pos_freq, int *slot_nat);
 
 /* Library version string, e.g. "sso 0.1 (sm_100a)". */
 const char *sso_version(void);

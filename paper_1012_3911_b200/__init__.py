@@ -27,7 +27,7 @@ OPT_GROUPS_PER_CTA, OPT_RING_BUFFERS, OPT_THREADS_PER_CTA, OPT_STRIDED_RING, OPT
 SYMBOLS = (
     "sso_plan_create", "sso_set_constants", "sso_set_potential", "sso_set_field", "sso_set_time_index",
     "sso_get_time_index", "sso_step", "sso_step_host", "sso_norm", "sso_set_option", "sso_launch_count",
-    "sso_destroy", "sso_last_error", "sso_version", "sso_debug_layout", "sso_profile_step", "sso_pass_name",
+    "sso_destroy", "sso_last_error", "sso_version", "sso_profile_step", "sso_pass_name",
     "sso_set_vector_potential", "sso_overlap", "sso_expect_position", "sso_expect_momentum", "sso_spectrum",
     "sso_filter_accumulate", "sso_step_observe", "sso_norm_static",
 )

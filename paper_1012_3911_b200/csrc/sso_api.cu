@@ -23,6 +23,7 @@
 #include <vector>
 
 #include "../../include/sso.h"
+#include "sso_debug.h"
 #include "sso_dispatch.h"
 #include "sso_line1d_args.h"
 
@@ -571,6 +572,7 @@ struct sso_plan {
     int opt_dirac_table = 0;
     int opt_tile_order = 0;   // SSO_OPT_TILE_ORDER
     int opt_cluster = 0;      // SSO_OPT_CLUSTER_1D
+    mutable int cl_fits[2] = {-1, -1};  // can this device co-schedule a cluster of 4 / 8 CTAs of the 1D kernel: -1 not asked yet
     struct ClusterLine {      // tables of the cluster version of the 1D kernel, built on first use for (cs, M = N / cs)
         int cs = 0, M = 0;
         void *tw = nullptr;       // twiddle blocks of the M-point transform
@@ -662,6 +664,14 @@ static void kinetic_layout(const sso_plan *p, int a, std::vector<double> &kv) {
     } else {
         kv = A.k_nat;
     }
+}
+
+// Device tables whose shape depends on the plan's configuration (the twiddle/frequency tables of the 1D cluster kernel,
+// the Dirac kinetic table of SSO_OPT_DIRAC_TABLE = 1).  Every call that changes the configuration -- sso_plan_create,
+// sso_set_option, sso_set_field, sso_set_vector_potential -- (re)allocates them here, so that sso_step itself only
+// enqueues kernels and can be captured into a CUDA graph on its very first call.
+namespace {
+int prepare_config_tables(sso_plan *plan);
 }
 
 extern "C" {
@@ -774,6 +784,7 @@ int sso_plan_create(sso_plan **out, int ndim, const int64_t *sizes, const double
         return rc;
     }
     int rc = sso_set_potential(plan, nullptr, 0, nullptr);
+    if (rc == SSO_OK) rc = prepare_config_tables(plan);
     if (rc != SSO_OK) {
         g_create_err = plan->err;
         sso_destroy(plan);
@@ -880,16 +891,20 @@ int sso_set_vector_potential(sso_plan *plan, const double *A, int on_device, voi
     if (!A) {
         cudaFree(plan->d_apos);
         plan->d_apos = nullptr;
-        return SSO_OK;
+        return prepare_config_tables(plan);
     }
     const size_t bytes = sizeof(double) * (size_t)plan->npts * plan->ndim;
+    // a host array is checked like the rows of sso_set_field; a device array is the caller's responsibility (sso.h)
+    if (!on_device)
+        for (size_t i = 0, cnt = (size_t)plan->npts * plan->ndim; i < cnt; ++i)
+            if (!isfinite(A[i])) return fail(plan, SSO_ERR_INVALID, "A holds a non-finite value");
     if (!plan->d_apos) {
         cudaError_t e = cudaMalloc((void **)&plan->d_apos, bytes);
         if (e != cudaSuccess) return fail(plan, SSO_ERR_ALLOC, std::string("vector potential: ") + cudaGetErrorString(e));
     }
     CK(cudaMemcpyAsync(plan->d_apos, A, bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
     CK(cudaStreamSynchronize(st));
-    return SSO_OK;
+    return prepare_config_tables(plan);
 }
 
 int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nvals) {
@@ -906,7 +921,7 @@ int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nval
         plan->kph_valid = false;
         plan->cl.kph_valid = false;
         plan->ktab_valid = false;
-        return SSO_OK;
+        return prepare_config_tables(plan);
     }
     if (!step_avg || nvals <= 0) return fail(plan, SSO_ERR_INVALID, "step_avg is NULL or nvals <= 0");
     const size_t cnt = (size_t)nvals * plan->ndim;
@@ -953,7 +968,7 @@ int sso_set_field(sso_plan *plan, int kind, const double *step_avg, int64_t nval
     plan->kph_valid = false;
     plan->cl.kph_valid = false;
     plan->ktab_valid = false;
-    return SSO_OK;
+    return prepare_config_tables(plan);
 }
 
 int sso_set_time_index(sso_plan *plan, int64_t n) {
@@ -1002,11 +1017,11 @@ int sso_set_option(sso_plan *plan, int option, int64_t value) {
                 plan->d_ktab = nullptr;
             }
             plan->ktab_valid = false;
-            return SSO_OK;
+            return prepare_config_tables(plan);
         case SSO_OPT_CLUSTER_1D:
             if (value != 0 && value != 1 && value != 4 && value != 8) return fail(plan, SSO_ERR_INVALID, "cluster mode must be 0 (auto), 1 (off), 4 or 8 (CTAs per cluster)");
             plan->opt_cluster = (int)value;
-            return SSO_OK;
+            return prepare_config_tables(plan);
         case SSO_OPT_TILE_ORDER:
             if (value < 0 || value > 16) return fail(plan, SSO_ERR_INVALID, "tile order must be in [0, 16]");
             plan->opt_tile_order = (int)value;
@@ -1565,10 +1580,7 @@ int build_ktab(sso_plan *plan, long long n, cudaStream_t st) {
     if (plan->ncomp == 1 || plan->ndim < 2 || !plan->opt_dirac_table) return SSO_OK;
     const bool shifted = plan->field_kind == SSO_FIELD_A;
     if (plan->ktab_valid && !shifted) return SSO_OK;
-    if (!plan->d_ktab) {
-        cudaError_t e = cudaMalloc(&plan->d_ktab, sizeof(double2) * (size_t)plan->npts);
-        if (e != cudaSuccess) return fail(plan, SSO_ERR_ALLOC, std::string("Dirac kinetic table: ") + cudaGetErrorString(e));
-    }
+    if (!plan->d_ktab) return fail(plan, SSO_ERR_STATE, "Dirac kinetic table missing (its allocation failed when the option was set)");
     double sh[3] = {0.0, 0.0, 0.0};
     if (shifted)
         for (int ax = 0; ax < plan->ndim; ++ax) sh[ax] = plan->charge * plan->h_avg[(size_t)n * plan->ndim + ax];
@@ -1589,7 +1601,22 @@ int build_ktab(sso_plan *plan, long long n, cudaStream_t st) {
 int cluster_size_for(const sso_plan *p) {
     if (p->ndim != 1 || p->ncomp != 1 || p->field_kind == SSO_FIELD_E || p->d_apos || p->opt_cluster == 1) return 0;
     const int n = p->ax[0].n;
-    auto usable = [&](int cs) { return n / cs >= 512 && n / cs <= SSO_MAX_LINE_CTA && find_line1d_cluster(p->precision, n / cs, cs) != nullptr; };
+    // built, and the current device can co-schedule cs CTAs with this much shared memory each (not a given on a MIG
+    // slice or a GPC with few SMs): asked once per plan and cluster size, cudaOccupancyMaxActiveClusters in the launcher
+    auto usable = [&](int cs) {
+        if (n / cs < 512 || n / cs > SSO_MAX_LINE_CTA) return false;
+        Line1dClusterLaunchFn lc = find_line1d_cluster(p->precision, n / cs, cs);
+        if (!lc) return false;
+        int &fits = p->cl_fits[cs == 8 ? 1 : 0];
+        if (fits < 0) {
+            const int M = n / cs;
+            const size_t smem = ((size_t)twiddle_count_padded(M) + (M + M / 16) + (line1d_cluster_alias(M) ? 0 : M) + (size_t)(cs - 1) * (M / cs)) * p->esize();
+            Line1dClusterArgs probe{};  // psi == NULL: occupancy query only, nothing is launched
+            fits = lc(probe, smem, nullptr) == cudaSuccess ? 1 : 0;
+            if (!fits) cudaGetLastError();
+        }
+        return fits == 1;
+    };
     if (p->opt_cluster > 1) return usable(p->opt_cluster) ? p->opt_cluster : 0;
     if (n > SSO_MAX_LINE_CTA) return usable(8) ? 8 : (usable(4) ? 4 : 0);
     return (n == SSO_MAX_LINE_CTA && usable(SSO_CLUSTER_AUTO_4096)) ? SSO_CLUSTER_AUTO_4096 : 0;
@@ -1640,6 +1667,19 @@ int build_cluster_tables(sso_plan *plan, int cs) {
     }
     cl.cs = cs;
     cl.M = M;
+    return SSO_OK;
+}
+
+int prepare_config_tables(sso_plan *plan) {
+    if (plan->ndim == 1) {
+        const int cs = cluster_size_for(plan);
+        return cs ? build_cluster_tables(plan, cs) : SSO_OK;  // a rebuilt ClusterLine starts with kph_valid = false
+    }
+    if (plan->opt_dirac_table && plan->ncomp > 1 && !plan->d_ktab) {
+        cudaError_t e = cudaMalloc(&plan->d_ktab, sizeof(double2) * (size_t)plan->npts);
+        if (e != cudaSuccess) return fail(plan, SSO_ERR_ALLOC, std::string("Dirac kinetic table: ") + cudaGetErrorString(e));
+        plan->ktab_valid = false;
+    }
     return SSO_OK;
 }
 
@@ -1750,7 +1790,10 @@ static int step_impl(sso_plan *plan, void *psi, int64_t nsteps, void *stream, Ob
         const int cs = cluster_size_for(plan);
         if (!cs && plan->ax[0].n > SSO_MAX_AXIS)
             return fail(plan, SSO_ERR_UNSUPPORTED, "1D lattices beyond 8192 points run on a thread-block cluster: Schroedinger without a length-gauge field only");
-        if (cs && (rc = build_cluster_tables(plan, cs)) != SSO_OK) return rc;
+        // the tables of the cluster kernel were made when the configuration was set (prepare_config_tables): nothing is
+        // allocated or copied here
+        if (cs && (plan->cl.cs != cs || plan->cl.M != plan->ax[0].n / cs))
+            return fail(plan, SSO_ERR_STATE, "cluster line tables missing (their allocation failed when the configuration was set)");
         for (long long s = 0; s < nsteps; s += chunk) {
             if (chunk > 0x7fffffffLL) return fail(plan, SSO_ERR_INVALID, "nsteps too large");
             if (cs) {
@@ -1993,6 +2036,9 @@ int sso_expect_momentum(sso_plan *plan, const void *psi, double *out_host, void 
     if (!psi || !out_host) return fail(plan, SSO_ERR_INVALID, "psi or out_host is NULL");
     if (((uintptr_t)psi & 15u) != 0) return fail(plan, SSO_ERR_INVALID, "psi must be 16-byte aligned");
     cudaStream_t st = (cudaStream_t)stream;
+    for (int a = 0; a < plan->ndim; ++a)
+        if (plan->ax[a].n > SSO_MAX_AXIS)
+            return fail(plan, SSO_ERR_UNSUPPORTED, "sso_expect_momentum: axes of at most 8192 points (longer 1D lattices exist only inside the cluster step kernel)");
     const size_t bytes = (size_t)plan->npts * plan->ncomp * plan->esize();
     if (!plan->d_scratch) {
         cudaError_t e = cudaMalloc(&plan->d_scratch, bytes);
@@ -2076,7 +2122,10 @@ int sso_step_observe(sso_plan *plan, void *psi, int64_t nsteps, const void *psi_
     if ((rc = sso_norm(plan, psi, &out_host[0], stream)) != SSO_OK) return rc;
     if (psi_ref && (rc = sso_overlap(plan, psi_ref, psi, &out_host[1], stream)) != SSO_OK) return rc;
     if ((rc = sso_expect_position(plan, psi, &out_host[3], stream)) != SSO_OK) return rc;
-    if (filter_acc && (rc = sso_filter_accumulate(plan, filter_acc, psi, filter_t, filter_T, filter_E, filter_dts, stream)) != SSO_OK) return rc;
+    if (filter_acc) {
+        if ((rc = sso_filter_accumulate(plan, filter_acc, psi, filter_t, filter_T, filter_E, filter_dts, stream)) != SSO_OK) return rc;
+        CK(cudaStreamSynchronize(st));  // the call returns with the stream drained on every path (sso.h)
+    }
     return SSO_OK;
 }
 

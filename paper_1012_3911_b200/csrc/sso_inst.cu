@@ -42,12 +42,20 @@ template <typename T, int N, bool STRIDED, int PW, int SIGN>
 cudaError_t launch_pass(const PassArgs &a, unsigned threads, size_t smem, cudaStream_t st) {
     auto kern = pass_kernel<T, N, STRIDED, PW, SIGN>;
     static std::atomic<unsigned long long> done{0};
-    int dev = 0, num_sms = 0;
-    cudaError_t e = opt_in_smem(kern, done, &dev, &num_sms);
+    int dev = 0;
+    cudaError_t e = opt_in_smem(kern, done, &dev);
     if (e != cudaSuccess) return e;
     // one wave of persistent CTAs: resident CTAs per SM for this block shape x SM count of the current device
-    int occ = 0;
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (int)threads, smem)) != cudaSuccess) return e;
+    // (asked once per device and block shape of this instantiation; the last answer is kept)
+    struct Occ { int dev; unsigned threads; size_t smem; int occ, sms; };
+    static thread_local Occ last{-1, 0u, 0, 0, 0};
+    if (last.dev != dev || last.threads != threads || last.smem != smem) {
+        int occ = 0, sms = 0;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (int)threads, smem)) != cudaSuccess) return e;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        last = Occ{dev, threads, smem, occ, sms};
+    }
+    const int occ = last.occ, num_sms = last.sms;
     if (occ < 1) return cudaErrorLaunchOutOfResources;
     long long grid = (long long)occ * num_sms;
     const long long need = ((long long)a.ntiles + a.G - 1) / a.G;
@@ -120,6 +128,11 @@ template <typename T, int M, int CS> cudaError_t launch_line1d_cluster(const Lin
     at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
+    if (!a.psi) {  // query only (sso_api.cu, cluster_size_for): can the current device hold one such cluster at all?
+        int nclusters = 0;
+        if ((e = cudaOccupancyMaxActiveClusters(&nclusters, kern, &cfg)) != cudaSuccess) return e;
+        return nclusters >= 1 ? cudaSuccess : cudaErrorLaunchOutOfResources;
+    }
     return cudaLaunchKernelEx(&cfg, kern, a);
 }
 

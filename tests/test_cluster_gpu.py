@@ -119,3 +119,38 @@ def test_8192_point_line_on_one_cta(torch):
     got, nrm, psi0 = run_gpu(torch, w, 6, sso.C64, 0, field=(sso.FIELD_E, np.ascontiguousarray(avg)))
     want = run_oracle(w, 6, psi0, field=(oracle.FIELD_E, avg))
     assert rel_l2(got, want) <= 2e-5
+
+
+def test_first_call_can_be_captured(torch):
+    """sso.h: sso_step only enqueues kernels from the first call on.  The tables of the cluster kernel (n = 4096 picks 8
+    CTAs by default) are made by sso_plan_create / sso_set_option, so the very first sso_step of a plan, and the first
+    one after the cluster choice changed, can sit inside a stream capture (cudaMalloc / cudaFree there would end it)."""
+    w = wl.config1(sizes=(4096,), nsteps=6)
+    want = run_oracle(w, 6, w.psi0)
+    for cluster in (0, 4, 1):
+        p = sso.Plan(w.sizes, w.dx, w.dt, 1, sso.C128)
+        p.set_potential(w.V)
+        p.set_option(sso.OPT_CLUSTER_1D, cluster)
+        psi = torch.from_numpy(w.psi0.copy()).cuda()
+        st = torch.cuda.Stream()
+        st.wait_stream(torch.cuda.current_stream())
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            p.step(psi, 3, stream=torch.cuda.current_stream())  # no warm-up call before the capture
+        g.replay()
+        g.replay()
+        torch.cuda.synchronize()
+        assert rel_l2(psi.cpu().numpy(), want) < TOL[sso.C128], cluster
+        p.destroy()
+
+
+def test_momentum_of_a_long_line_is_refused_up_front(torch):
+    """sso_expect_momentum has no transform beyond 8192 points: SSO_ERR_UNSUPPORTED, stated in sso.h, before any work."""
+    w = wl.config1(sizes=(16384,), nsteps=1)
+    p = sso.Plan(w.sizes, w.dx, w.dt, 1, sso.C128)
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    with pytest.raises(sso.SsoError) as ei:
+        p.expect_momentum(psi)
+    assert ei.value.code == sso.ERR_UNSUPPORTED
+    assert abs(p.norm(psi) - 1.0) < 1e-12  # the plan is still usable
+    p.destroy()

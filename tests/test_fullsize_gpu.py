@@ -286,7 +286,7 @@ def test_steps_on_a_side_stream_and_graph_capture(torch):
     st = torch.cuda.Stream()
     st.wait_stream(torch.cuda.current_stream())
     with torch.cuda.stream(st):
-        p.step(psi, 2, stream=st)  # warm-up builds the static tables outside the capture
+        p.step(psi, 2, stream=st)
     st.synchronize()
     g = torch.cuda.CUDAGraph()
     p.set_time_index(2)
@@ -295,4 +295,22 @@ def test_steps_on_a_side_stream_and_graph_capture(torch):
     g.replay()
     torch.cuda.synchronize()
     assert rel_l2(psi.cpu().numpy(), oracle_steps(w, 5)) < 1e-13
+    p.destroy()
+
+
+def test_first_step_of_a_dirac_table_plan_can_be_captured(torch):
+    """SSO_OPT_DIRAC_TABLE = 1: the table is allocated by sso_set_option, not by the first sso_step, which therefore
+    can sit inside a stream capture without a warm-up call (only the kernel that fills the table is enqueued)."""
+    w = wl.config4(sizes=(64, 64), nsteps=4)
+    p = make_plan(w)
+    p.set_option(sso.OPT_DIRAC_TABLE, 1)
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=st):
+        p.step(psi, 4, stream=torch.cuda.current_stream())
+    g.replay()
+    torch.cuda.synchronize()
+    assert rel_l2(psi.cpu().numpy(), oracle_steps(w, 4)) < 1e-12
     p.destroy()

@@ -217,6 +217,15 @@ def test_position_space_vector_potential(torch):
     with pytest.raises(sso.SsoError) as e:
         sso.Plan((64,), (0.1,), 0.01, 1).set_vector_potential(np.ones((1, 64)))
     assert e.value.code == sso.ERR_UNSUPPORTED
+    # a host array with a NaN or an Inf is refused like the rows of sso_set_field (it would end up in psi otherwise)
+    p = sso.Plan((32, 32), (0.1, 0.1), 0.01, 2)
+    for bad in (np.nan, np.inf):
+        A = np.zeros((2, 32, 32))
+        A[1, 7, 5] = bad
+        with pytest.raises(sso.SsoError) as e:
+            p.set_vector_potential(A)
+        assert e.value.code == sso.ERR_INVALID
+    p.destroy()
 
 
 def test_field_e_on_every_axis(torch):
