@@ -9,13 +9,15 @@ sso_step(psi, SPLIT_STEPS) that advances the wavefunction by SPLIT_STEPS = 128 s
 
 Headline workload at N=1: BASELINE.json's metric is not quoted on one config, so the line's top-level numbers are
 for the LARGEST single-GPU configuration, config 5 (3D Dirac, 4 x 256^3 complex128, 1 GiB of psi); the other
-workloads (1, 2a, 2b, 3, 4, and the paper's 1D Dirac and 4-component 2D Dirac shapes d1, d2x4, d2A) are timed in the same run and reported under config.per_workload.
+workloads (1, 2a, 2b, 3, 4, and the paper's 1D Dirac and 4-component 2D Dirac shapes d1, d2x4, d2A) are timed in the same
+run and reported under config.per_workload and, flat, as config.us_<name> / frac8_<name> / fracM_<name>.
   value  device-resident throughput: psi, the potential table and the field table are in HBM before the
          timed region; K calls timed with CUDA events on the launching stream.
   e2e    the same K calls through sso_step_host on a pinned HOST buffer: every call uploads psi, steps and
          downloads it inside the timed region.
   roofline  HBM: algorithmic bytes of one pass-kernel launch (one read + one write of psi, DESIGN.md
          "Rooflines") / average pass-kernel launch duration over the timed region, against MEASURED_PEAKS.json;
+         `frac_dominant` = 2 S / mean launch time of the pass kind that takes most of a step / peak;
          `per_pass` = the same for each pass kind of one split step, timed with CUDA events by the library
          (sso_profile_step); `traffic` = ncu DRAM bytes of the dominant kernel from profiles/traffic.json, or
          null when csrc/ has changed since that capture.
@@ -226,13 +228,28 @@ def run_reference(args):
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": DESCR[name], "split_steps_per_step": REF_SPLIT, "grid": list(w.sizes), "ncomp": w.ncomp},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle", "sample": sample},
+        # the same descriptive keys and values as the product arm (the workload is the same; that a bench step here is a
+        # sample of REF_SPLIT of its 128 split-operator steps is said under cpu_baseline.sample)
+        "config": describe_config(name, w, prec, int(os.environ.get("WORLD_SIZE", "1"))),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle", "sample": sample,
+                         "split_steps_per_bench_step": REF_SPLIT},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
     return 0
+
+
+def l2_note(S: float) -> str:
+    return ("psi larger than L2: every pass streams it from HBM" if S > 126e6 else
+            "psi (%.0f MB) fits L2 (126 MB): consecutive passes of a step sequence re-touch it there; no flush, ncu DRAM bytes are below the algorithmic bytes" % (S / 1e6))
+
+
+def describe_config(name, w, prec, world):
+    """The keys of `config` that name the workload: identical in the product and the reference arm."""
+    S = w.npoints * w.ncomp * (16 if prec == "c128" else 8)
+    return {"workload": DESCR[name], "split_steps_per_step": SPLIT_STEPS, "grid": list(w.sizes), "ncomp": w.ncomp,
+            "parallelism": "replicas" if world > 1 else "single GPU", "l2": l2_note(S)}
 
 
 def job_throughput(updates_per_rank: float, ms_local: float, world: int, device: str = "cuda"):
@@ -308,8 +325,7 @@ def measure(name, K, W, world, barrier, sampler, want_e2e):
         "achieved_GBs": achieved, "frac_of_measured": achieved / peak, "frac_of_8TBs": achieved / 8000.0,
         "bar_us_per_split_step": BAR_US[name], "meets_60pct_of_8TBs": (us_step <= BAR_US[name]) if BAR_US[name] else None,
         "norm_after": norm_after, "clocks": clocks, "gpu_launches": int(launches_per_call * K),
-        "l2": ("psi larger than L2: every pass streams it from HBM" if S > 126e6 else
-               "psi (%.0f MB) fits L2 (126 MB): consecutive passes of a step sequence re-touch it there; no flush, ncu DRAM bytes are below the algorithmic bytes" % (S / 1e6)),
+        "l2": l2_note(S),
     }
     if nd == 1:
         rec["note"] = "one persistent CTA, psi stays on the SM for all 128 steps: the HBM figure is 2S per CALL over the call time, not a roofline (SURVEY H5)"
@@ -384,16 +400,28 @@ def run_product(args):
         traffic, traffic_src = ncu_traffic(head)
         nd = len(w.sizes)
         dominant = max(rec.get("per_pass", []), key=lambda r: r["avg_us"] * r["launches"], default=None)
+        # the dominant pass KIND's own fraction: 2 S over its mean launch time (events around each launch of a profiled
+        # step sequence), next to the step average `frac`
+        dom_gbs = bytes_per_launch / (dominant["avg_us"] * 1e-6) / 1e9 if (dominant and dominant["avg_us"] > 0 and nd > 1) else None
+        cfg = describe_config(head, w, "c128" if rec["dtype"] == "f64" else "c64", world)
+        cfg.update({"us_per_split_step": rec["us_per_split_step"], "norm_after": rec["norm_after"]})
+        # one flat scalar per workload (records that keep only the scalar keys of `config` still carry every workload):
+        # us per split step, fraction of the 8 TB/s roofline and of the measured copy bandwidth (None in 1D: psi stays on the SM)
+        for nm, r in per.items():
+            cfg[f"us_{nm}"] = round(r["us_per_split_step"], 3)
+            cfg[f"frac8_{nm}"] = round(r["frac_of_8TBs"], 4) if r["frac_of_8TBs"] is not None else None
+            cfg[f"fracM_{nm}"] = round(r["frac_of_measured"], 4) if r["frac_of_measured"] is not None else None
+        cfg["per_workload"] = per
         line = {
             "metric": METRIC, "value": rec["updates_per_s"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": rec["dtype"], "data": "synthetic",
-            "config": {"workload": DESCR[head], "split_steps_per_step": SPLIT_STEPS, "grid": list(w.sizes), "ncomp": w.ncomp,
-                       "parallelism": "replicas" if world > 1 else "single GPU", "us_per_split_step": rec["us_per_split_step"],
-                       "l2": rec["l2"], "norm_after": rec["norm_after"], "per_workload": per},
+            "config": cfg,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                          "traffic_source": traffic_src,
                          "kernel": ("average over the pass launches of a split step (every pass launch moves psi once: sso::ring_kernel on the contiguous axis, sso::sring_kernel on the strided axes); per_pass lists each" if nd > 1 else "sso::pass_kernel (one persistent CTA, psi stays on the SM)"),
-                         "dominant_pass": dominant, "bytes_per_launch": bytes_per_launch, "avg_launch_us": per_launch_s * 1e6,
+                         "dominant_pass": dominant, "dominant_achieved": dom_gbs,
+                         "frac_dominant": dom_gbs / peak if dom_gbs else None,
+                         "frac_dominant_of_nominal_8TBs": dom_gbs / 8000.0 if dom_gbs else None, "bytes_per_launch": bytes_per_launch, "avg_launch_us": per_launch_s * 1e6,
                          "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
             "e2e": e2e,
             "gpu_launches": rec["gpu_launches"],
