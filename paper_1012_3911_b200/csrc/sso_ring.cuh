@@ -147,9 +147,11 @@ struct TileRing {
     // group leader: draw the group's next ticket; the group barrier that follows publishes it
     __device__ void draw(int grp) const { mail[grp] = atomicAdd(ticket, 1); }
     __device__ int drawn(int grp) const { return mail[grp]; }
-    // blocks until tile s (< nloc) has landed; returns its buffer
+    // blocks until tile s (< nloc) has landed; returns its buffer.  The poll for a fill that has not been issued yet
+    // is bounded: a tile of this CTA is issued within a pass (milliseconds), so 2^27 polls of >= 64 ns each (> 8 s)
+    // mean the protocol is broken, and the kernel traps (the launch then fails with an error) instead of hanging.
     __device__ int wait(int s) const {
-        for (;;) {
+        for (unsigned polls = 0;; ++polls) {
             for (int b = 0; b < NB; ++b) {
                 const int v = tag[b];
                 if ((v >> 1) == s + 1) {
@@ -157,6 +159,7 @@ struct TileRing {
                     return b;
                 }
             }
+            if (polls >> 27) __trap();
             __nanosleep(64);  // the load of tile s has not been issued yet
         }
     }
