@@ -314,3 +314,33 @@ def test_first_step_of_a_dirac_table_plan_can_be_captured(torch):
     torch.cuda.synchronize()
     assert rel_l2(psi.cpu().numpy(), oracle_steps(w, 4)) < 1e-12
     p.destroy()
+
+
+BENCH_ONLY = [
+    ("d1", lambda: wl.dirac1d(sizes=(4096,), nsteps=100, ncomp=2), 100),
+    ("d2x4", lambda: wl.dirac2d4(nsteps=20), 20),
+    ("d2A", lambda: wl.dirac2d_magnetic(nsteps=20), 20),
+]
+
+
+@pytest.mark.parametrize("name,make,nsteps", BENCH_ONLY, ids=[b[0] for b in BENCH_ONLY])
+def test_bench_only_workloads_at_full_size(torch, name, make, nsteps):
+    """The three workloads bench.py times besides BASELINE.json's configs (the paper's 1D Dirac line, its 4-component
+    2D Dirac shape, and 2D Dirac with A(r) applied in position space, eq. 26), at the size and in the launch
+    configuration of the bench (default options, one call), element by element against the oracle."""
+    w = make()
+    p = make_plan(w)
+    o = make_oracle(w)
+    if "A" in w.extra:
+        p.set_vector_potential(np.ascontiguousarray(w.extra["A"]))
+        o.set_vector_potential(w.extra["A"])
+    psi = torch.from_numpy(w.psi0.copy()).cuda()
+    p.step(psi, nsteps)
+    torch.cuda.synchronize()
+    nrm = p.norm(psi)
+    p.destroy()
+    got = psi.cpu().numpy()
+    want = o.step(w.psi0.astype(np.complex128), nsteps)
+    assert rel_l2(got, want) <= TOL[sso.C128], (name, rel_l2(got, want))
+    assert np.abs(got - want).max() <= 5 * TOL[sso.C128] * np.abs(want).max(), name
+    assert abs(nrm - 1.0) < 1e-11
